@@ -1,0 +1,98 @@
+"""ORACLE -- TEST INFRASTRUCTURE ONLY (see chase_filter_oracle.c for the full header).
+
+ctypes front end to the plain-C FP64 oracle of the ChASE Chebyshev filter
+(Alg. 4, Eq. (7)).  It imports nothing from the
+product package and the product package imports nothing from here.  Allowed callers:
+tests/, __graft_entry__.smoke(), bench.py's cpu_baseline / --impl reference legs.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_DIR = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_DIR, "chase_filter_oracle.c")
+_LIB = os.path.join(_DIR, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp; no -march so the same .so runs on any x86-64 host."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-Wall",
+                               "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_chase_scalars.restype = None
+        lib.oracle_chase_scalars.argtypes = [ctypes.c_double] * 3 + [ctypes.c_int] + [ctypes.c_void_p] * 5
+        lib.oracle_chase_filter.restype = ctypes.c_int
+        lib.oracle_chase_filter.argtypes = [
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int64,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p,
+            ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def chase_scalars(a: float, b: float, lambda1: float, m_max: int):
+    """(sigma[1..m], alpha[1..m], beta[1..m], c, e) of Alg. 4; arrays have length m_max+1, entry 0 unused."""
+    lib = _load()
+    sigma = np.zeros(m_max + 1)
+    alpha = np.zeros(m_max + 1)
+    beta = np.zeros(m_max + 1)
+    c = ctypes.c_double()
+    e = ctypes.c_double()
+    lib.oracle_chase_scalars(a, b, lambda1, m_max, sigma.ctypes.data, alpha.ctypes.data,
+                             beta.ctypes.data, ctypes.addressof(c), ctypes.addressof(e))
+    return sigma, alpha, beta, c.value, e.value
+
+
+def chase_filter(H: np.ndarray, V0: np.ndarray, degrees, a: float, b: float, lambda1: float) -> np.ndarray:
+    """out[:, j] = p_{degrees[j]}(H) V0[:, j], FP64, returned as a new Fortran-ordered array.
+
+    H: N x N, Fortran-contiguous, dtype float64/complex128 (used as is) or
+       float32/complex64 (upcast element-wise inside the C loop).
+    V0: N x ncols, any float/complex dtype; upcast to FP64 (complex iff H is complex).
+    """
+    lib = _load()
+    H = np.asarray(H)
+    if H.ndim != 2 or H.shape[0] != H.shape[1]:
+        raise ValueError("H must be square")
+    if not H.flags.f_contiguous:
+        H = np.asfortranarray(H)
+    is_complex = np.iscomplexobj(H)
+    h_is_f32 = H.dtype in (np.float32, np.complex64)
+    if H.dtype not in (np.float32, np.float64, np.complex64, np.complex128):
+        raise ValueError(f"unsupported H dtype {H.dtype}")
+    N = H.shape[0]
+    wide = np.complex128 if is_complex else np.float64
+    if np.iscomplexobj(V0) and not is_complex:
+        raise ValueError("complex V0 with real H")
+    V = np.array(V0, dtype=wide, order="F", copy=True)
+    if V.ndim != 2 or V.shape[0] != N:
+        raise ValueError("V0 must be N x ncols")
+    W = np.empty_like(V, order="F")
+    deg = np.ascontiguousarray(np.asarray(degrees, dtype=np.int32))
+    if deg.shape != (V.shape[1],):
+        raise ValueError("degrees must have one entry per column")
+    rc = lib.oracle_chase_filter(H.ctypes.data, int(h_is_f32), int(is_complex), N,
+                                 V.ctypes.data, W.ctypes.data, V.shape[1], deg.ctypes.data,
+                                 float(a), float(b), float(lambda1))
+    if rc != 0:
+        raise RuntimeError(f"oracle_chase_filter failed: {rc}")
+    return V
