@@ -1,0 +1,124 @@
+/*
+ * chase_filter.h -- C ABI of the B200-native Chebyshev polynomial filter of ChASE
+ * (arXiv 1805.10121).  Plain pointers and sizes only; no torch / C++ types.
+ *
+ * Operation (Alg. 4 "Chebyshev filter for optimized even degrees";
+ * PAPER.md:311-313 Eq. (7); Eq. (5)):
+ *
+ *     V[:, j]  <-  p_{m_j}(H) V[:, j],     m_j = degrees[j],   j = 0 .. ncols-1
+ *     p_m(x) = C_m((x - c)/e) / C_m((lambda1 - c)/e),  c = (a+b)/2,  e = (b-a)/2
+ *
+ * evaluated by the scaled three-term recurrence
+ *     V_1     = (sigma_1/e) (H - cI) V_0
+ *     V_{k+1} = (2 sigma_{k+1}/e) (H - cI) V_k - sigma_k sigma_{k+1} V_{k-1}
+ *     sigma_1 = e/(lambda1 - c),  sigma_{k+1} = 1/(2/sigma_1 - sigma_k)
+ * with a = mu_{nev+nex}, b = b_sup, lambda1 = mu_1.  Columns are sorted by
+ * ascending degree (Alg. 1 l.15) so that step k works on the contiguous
+ * suffix of columns with m_j >= k: one kernel launch, one pass over H per
+ * step; shift (-c V_k), scaling and the V_{k-1} term are fused into the kernel epilogue
+ * (replaces the paper's Shift + HEMM, Listing 1/2).
+ *
+ * Layouts (Listing 2): all matrices COLUMN-MAJOR, leading dimension N;
+ * complex = interleaved (re, im) like std::complex<T>.  H is N x N, FULL Hermitian storage
+ * (both triangles; read as a general matrix), never written.  V is N x ncols.
+ *
+ * Degrees: any m_j >= 0, non-decreasing.  0 leaves the column untouched, odd values are
+ * accepted (the paper emits even ones only so that the result lands in V without a copy,
+ * PAPER.md:393; here an odd-degree column costs one device copy of that column).
+ *
+ * All calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = legacy
+ * default stream) unless stated otherwise.  The library never frees or retains caller
+ * memory; `degrees` (HOST) is consumed before the call returns; H, V, workspace must stay
+ * alive until `stream` has drained.
+ *
+ * Return codes: 0 success; negative = rejected before any launch (CHASE_ERR_*);
+ * positive = a cudaError_t from a failed allocation / launch / copy.
+ * ncols == 0 or max(degrees) == 0 is a success that launches nothing.
+ */
+#ifndef CHASE_FILTER_H
+#define CHASE_FILTER_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CHASE_F32 = 0,  /* float,                 FP32 FMA arithmetic */
+    CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N % 16 == 0) */
+    CHASE_C64 = 2,  /* interleaved float2,    FP32 FMA arithmetic */
+    CHASE_C128 = 3  /* interleaved double2,   FP64 (DMMA tensor path when N % 8 == 0) */
+} chase_dtype_t;
+
+enum {
+    CHASE_OK = 0,
+    CHASE_ERR_ARG = -1,       /* null pointer, N <= 0, ncols < 0, N or ncols too large */
+    CHASE_ERR_BOUNDS = -2,    /* not (lambda1 < a < b), or a non-finite bound (reading G8) */
+    CHASE_ERR_DEGREES = -3,   /* a negative degree, or degrees not non-decreasing (G7) */
+    CHASE_ERR_DTYPE = -4,     /* unknown chase_dtype_t */
+    CHASE_ERR_WORKSPACE = -5, /* workspace null or smaller than chase_filter_workspace_bytes */
+    CHASE_ERR_ALIGN = -6      /* H, V or workspace not aligned to 16 bytes */
+};
+
+/* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype`
+ * (the W of Alg. 4), rounded up to 256 bytes.  0 if an argument is invalid. */
+size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
+
+/* The filter with caller-provided scratch.
+ *   H          DEVICE, N x N column-major, ld = N, 16-byte aligned, read-only
+ *   V          DEVICE, N x ncols column-major, ld = N, 16-byte aligned; in: V_0, out: result
+ *   degrees    HOST, int32[ncols], non-decreasing, each >= 0
+ *   a, b, lambda1   real bounds, lambda1 < a < b, finite (also for complex dtypes)
+ *   workspace  DEVICE, >= chase_filter_workspace_bytes(...) bytes, 16-byte aligned; contents
+ *              undefined on entry and exit
+ *   stream     cudaStream_t
+ * Enqueues exactly max(degrees) step kernels (plus one small copy kernel if any degree is
+ * odd) and returns without synchronising. */
+int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                    double a, double b, double lambda1, chase_dtype_t dtype,
+                    void *workspace, size_t workspace_bytes, void *stream);
+
+/* Same, scratch taken with cudaMallocAsync / cudaFreeAsync on `stream`. */
+int chase_filter(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                 double a, double b, double lambda1, chase_dtype_t dtype, void *stream);
+
+/* End-to-end convenience for callers whose data lives on the HOST: H and V are HOST
+ * pointers (pinned or pageable).  Allocates device buffers, copies H and V to the device,
+ * runs chase_filter_ws, copies V back, frees, and SYNCHRONISES before returning.
+ * `device` is the CUDA device ordinal. */
+int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols,
+                      const int32_t *degrees, double a, double b, double lambda1,
+                      chase_dtype_t dtype, int device);
+
+/* Host-side pieces of Alg. 4, exposed for tests and callers that want to inspect the plan.
+ * chase_filter_scalars: alpha[k], beta[k] (k = 1..m_max; entry 0 unused; arrays of m_max+1
+ *   doubles, HOST) such that V_k = alpha[k] (H - cI) V_{k-1} + beta[k] V_{k-2}; *c = center.
+ *   (Alg. 4 l.2-5, 8, 11.)  Returns 0 or CHASE_ERR_BOUNDS / CHASE_ERR_ARG.
+ * chase_filter_schedule: offset[k] (k = 1..m_max, entry 0 unused; HOST int32[m_max+1]) =
+ *   first active column of step k = #{j : degrees[j] < k} (Alg. 4 l.12-14).  Returns m_max
+ *   (>= 0) or CHASE_ERR_DEGREES / CHASE_ERR_ARG; pass offset = NULL to only get m_max. */
+int chase_filter_scalars(double a, double b, double lambda1, int32_t m_max,
+                         double *alpha, double *beta, double *c);
+int chase_filter_schedule(const int32_t *degrees, int64_t ncols, int32_t *offset);
+
+/* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel,
+ * 0 = generic FMA kernel.  Negative = invalid arguments. */
+int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
+
+/* Number of kernels launched by this library since load (all streams); for bench.py. */
+int64_t chase_filter_launch_count(void);
+
+/* Register-only FP64 peak probes on the current device (synchronous; for the roofline
+ * denominator in bench.py).  kind 0: dependent-free DFMA chains, kind 1: mma.sync m8n8k4
+ * f64 (SASS DMMA.8x8x4) chains.  Writes achieved GFLOP/s over `iters` inner iterations on
+ * all SMs.  Returns 0 or a cudaError_t. */
+int chase_fp64_peak_probe(int kind, int iters, double *gflops);
+
+const char *chase_filter_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CHASE_FILTER_H */

@@ -1,0 +1,208 @@
+"""Thin ctypes binding of libchase_filter.so (include/chase_filter.h): argument marshalling
+only.  Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for
+device memory and streams.  There is no CPU fallback: a missing library raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+from . import _build
+
+CHASE_F32, CHASE_F64, CHASE_C64, CHASE_C128 = 0, 1, 2, 3
+_DTYPE_CODE = {torch.float32: CHASE_F32, torch.float64: CHASE_F64,
+               torch.complex64: CHASE_C64, torch.complex128: CHASE_C128}
+
+EXPORTS = [
+    "chase_filter", "chase_filter_ws", "chase_filter_host", "chase_filter_workspace_bytes",
+    "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
+    "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror",
+]
+
+_lib = None
+
+
+class ChaseFilterError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"chase_filter error {code}: {msg}")
+        self.code = code
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load() -> ctypes.CDLL:
+    """Load the in-tree shared library; fail loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise ImportError(
+            f"{path} is missing: build it with `python -m paper_1805_10121_b200._build` "
+            "(or __graft_entry__.build()).  There is no CPU fallback.")
+    lib = ctypes.CDLL(path)
+    vp, i64, i32, dbl, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_size_t
+    lib.chase_filter_workspace_bytes.restype = sz
+    lib.chase_filter_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
+    lib.chase_filter_ws.restype = ctypes.c_int
+    lib.chase_filter_ws.argtypes = [vp, i64, vp, i64, vp, dbl, dbl, dbl, ctypes.c_int, vp, sz, vp]
+    lib.chase_filter.restype = ctypes.c_int
+    lib.chase_filter.argtypes = [vp, i64, vp, i64, vp, dbl, dbl, dbl, ctypes.c_int, vp]
+    lib.chase_filter_host.restype = ctypes.c_int
+    lib.chase_filter_host.argtypes = [vp, i64, vp, i64, vp, dbl, dbl, dbl, ctypes.c_int, ctypes.c_int]
+    lib.chase_filter_scalars.restype = ctypes.c_int
+    lib.chase_filter_scalars.argtypes = [dbl, dbl, dbl, i32, vp, vp, vp]
+    lib.chase_filter_schedule.restype = ctypes.c_int
+    lib.chase_filter_schedule.argtypes = [vp, i64, vp]
+    lib.chase_filter_kernel_path.restype = ctypes.c_int
+    lib.chase_filter_kernel_path.argtypes = [i64, i64, ctypes.c_int]
+    lib.chase_filter_launch_count.restype = i64
+    lib.chase_filter_launch_count.argtypes = []
+    lib.chase_fp64_peak_probe.restype = ctypes.c_int
+    lib.chase_fp64_peak_probe.argtypes = [ctypes.c_int, ctypes.c_int, vp]
+    lib.chase_filter_strerror.restype = ctypes.c_char_p
+    lib.chase_filter_strerror.argtypes = [ctypes.c_int]
+    _lib = lib
+    return lib
+
+
+def chase_filter_strerror(code: int) -> str:
+    return load().chase_filter_strerror(int(code)).decode()
+
+
+def _check(code: int) -> None:
+    if code != 0:
+        raise ChaseFilterError(code, chase_filter_strerror(code))
+
+
+def _degrees_array(degrees, ncols: int) -> np.ndarray:
+    if isinstance(degrees, torch.Tensor):
+        degrees = degrees.cpu().numpy()
+    deg = np.ascontiguousarray(np.asarray(degrees, dtype=np.int32))
+    if deg.shape != (ncols,):
+        raise ValueError(f"degrees must have shape ({ncols},), got {deg.shape}")
+    return deg
+
+
+def _check_colmajor(x: torch.Tensor, name: str) -> None:
+    if x.dim() != 2 or (x.shape[0] > 1 and x.stride(0) != 1) or \
+            (x.shape[1] > 1 and x.stride(1) != x.shape[0]):
+        raise ValueError(f"{name} must be column-major with ld = rows "
+                         f"(shape {tuple(x.shape)}, strides {x.stride()})")
+
+
+def _stream_ptr(stream: Optional[torch.cuda.Stream]) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def chase_filter_workspace_bytes(N: int, ncols: int, dtype: torch.dtype) -> int:
+    return int(load().chase_filter_workspace_bytes(N, ncols, _DTYPE_CODE[dtype]))
+
+
+def chase_filter_kernel_path(N: int, ncols: int, dtype: torch.dtype) -> int:
+    return int(load().chase_filter_kernel_path(N, ncols, _DTYPE_CODE[dtype]))
+
+
+def chase_filter_launch_count() -> int:
+    return int(load().chase_filter_launch_count())
+
+
+def chase_filter_ws(H: torch.Tensor, V: torch.Tensor, degrees, a: float, b: float, lambda1: float,
+                    workspace: torch.Tensor, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """V[:, j] <- p_{degrees[j]}(H) V[:, j] in place (device tensors, column-major).
+    `workspace`: any device tensor of >= chase_filter_workspace_bytes bytes.  Asynchronous."""
+    lib = load()
+    if not (H.is_cuda and V.is_cuda and workspace.is_cuda):
+        raise ValueError("H, V and workspace must be CUDA tensors (there is no CPU path)")
+    if H.dtype != V.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V, "V")
+    N, ncols = V.shape
+    if H.shape != (N, N):
+        raise ValueError("H must be N x N with N = V.shape[0]")
+    deg = _degrees_array(degrees, ncols)
+    ws_bytes = workspace.numel() * workspace.element_size()
+    with torch.cuda.device(H.device):
+        rc = lib.chase_filter_ws(H.data_ptr(), N, V.data_ptr(), ncols, deg.ctypes.data,
+                                 float(a), float(b), float(lambda1), _DTYPE_CODE[H.dtype],
+                                 workspace.data_ptr(), ws_bytes, _stream_ptr(stream))
+    _check(rc)
+    return V
+
+
+def chase_filter(H: torch.Tensor, V: torch.Tensor, degrees, a: float, b: float, lambda1: float,
+                 stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """Same as chase_filter_ws; scratch comes from cudaMallocAsync inside the library."""
+    lib = load()
+    if not (H.is_cuda and V.is_cuda):
+        raise ValueError("H and V must be CUDA tensors (there is no CPU path)")
+    if H.dtype != V.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V, "V")
+    N, ncols = V.shape
+    if H.shape != (N, N):
+        raise ValueError("H must be N x N with N = V.shape[0]")
+    deg = _degrees_array(degrees, ncols)
+    with torch.cuda.device(H.device):
+        rc = lib.chase_filter(H.data_ptr(), N, V.data_ptr(), ncols, deg.ctypes.data,
+                              float(a), float(b), float(lambda1), _DTYPE_CODE[H.dtype],
+                              _stream_ptr(stream))
+    _check(rc)
+    return V
+
+
+def chase_filter_host(H: torch.Tensor, V: torch.Tensor, degrees, a: float, b: float, lambda1: float,
+                      device: int = 0) -> torch.Tensor:
+    """HOST tensors in, result in V (host); H2D/D2H copies happen inside the C call."""
+    lib = load()
+    if H.is_cuda or V.is_cuda:
+        raise ValueError("chase_filter_host takes host tensors")
+    if H.dtype != V.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V, "V")
+    N, ncols = V.shape
+    deg = _degrees_array(degrees, ncols)
+    rc = lib.chase_filter_host(H.data_ptr(), N, V.data_ptr(), ncols, deg.ctypes.data,
+                               float(a), float(b), float(lambda1), _DTYPE_CODE[H.dtype], int(device))
+    _check(rc)
+    return V
+
+
+def chase_filter_scalars(a: float, b: float, lambda1: float, m_max: int):
+    """(alpha[0..m_max], beta[0..m_max], c); entry 0 unused."""
+    alpha = np.zeros(m_max + 1)
+    beta = np.zeros(m_max + 1)
+    c = ctypes.c_double()
+    _check(load().chase_filter_scalars(float(a), float(b), float(lambda1), int(m_max),
+                                       alpha.ctypes.data, beta.ctypes.data, ctypes.addressof(c)))
+    return alpha, beta, c.value
+
+
+def chase_filter_schedule(degrees: Sequence[int]):
+    """(m_max, offset[0..m_max]) with offset[k] = first active column of step k."""
+    deg = np.ascontiguousarray(np.asarray(degrees, dtype=np.int32))
+    lib = load()
+    m_max = lib.chase_filter_schedule(deg.ctypes.data, deg.size, None)
+    if m_max < 0:
+        _check(m_max)
+    offset = np.zeros(m_max + 1, dtype=np.int32)
+    lib.chase_filter_schedule(deg.ctypes.data, deg.size, offset.ctypes.data)
+    return m_max, offset
+
+
+def chase_fp64_peak_probe(kind: int, iters: int = 4096) -> float:
+    """GFLOP/s of the register-only probe (0: DFMA, 1: DMMA.8x8x4) on the current device."""
+    g = ctypes.c_double()
+    _check(load().chase_fp64_peak_probe(int(kind), int(iters), ctypes.addressof(g)))
+    return g.value

@@ -1,0 +1,238 @@
+// Host orchestration of the Chebyshev filter (Alg. 4) behind the C ABI of
+// include/chase_filter.h: validation, the sigma recurrence (l.2-5, 8, 11), the active-suffix
+// schedule (l.12-14) and one fused step kernel per degree on one CUDA stream.
+#include <atomic>
+#include <cmath>
+#include <cstdlib>
+#include <vector>
+
+#include "chase_internal.h"
+
+namespace chase {
+static std::atomic<int64_t> g_launches{0};
+void count_launch() { g_launches.fetch_add(1, std::memory_order_relaxed); }
+
+static size_t elem_bytes(chase_dtype_t dtype) {
+    switch (dtype) {
+        case CHASE_F32: return 4;
+        case CHASE_F64: return 8;
+        case CHASE_C64: return 8;
+        case CHASE_C128: return 16;
+        default: return 0;
+    }
+}
+static const int64_t kMaxDim = (int64_t)1 << 30;   // keeps every index product inside int64
+}  // namespace chase
+
+using namespace chase;
+
+extern "C" {
+
+const char *chase_filter_strerror(int code) {
+    switch (code) {
+        case CHASE_OK: return "success";
+        case CHASE_ERR_ARG: return "invalid argument (null pointer or bad size)";
+        case CHASE_ERR_BOUNDS: return "bounds must satisfy lambda1 < a < b and be finite";
+        case CHASE_ERR_DEGREES: return "degrees must be >= 0 and non-decreasing";
+        case CHASE_ERR_DTYPE: return "unknown dtype";
+        case CHASE_ERR_WORKSPACE: return "workspace missing or too small";
+        case CHASE_ERR_ALIGN: return "H, V and workspace must be 16-byte aligned";
+        default:
+            if (code > 0) return cudaGetErrorString((cudaError_t)code);
+            return "unknown error";
+    }
+}
+
+int64_t chase_filter_launch_count(void) { return g_launches.load(); }
+
+size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype) {
+    size_t w = elem_bytes(dtype);
+    if (w == 0 || N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return 0;
+    size_t bytes = (size_t)N * (size_t)ncols * w;
+    return (bytes + 255) / 256 * 256;
+}
+
+int chase_filter_scalars(double a, double b, double lambda1, int32_t m_max,
+                         double *alpha, double *beta, double *c_out) {
+    if (m_max < 0 || (m_max > 0 && (!alpha || !beta))) return CHASE_ERR_ARG;
+    if (!(std::isfinite(a) && std::isfinite(b) && std::isfinite(lambda1))) return CHASE_ERR_BOUNDS;
+    if (!(lambda1 < a && a < b)) return CHASE_ERR_BOUNDS;
+    const double c = 0.5 * (b + a);               // Alg. 4 l.2
+    const double e = 0.5 * (b - a);               // l.2
+    const double sigma1 = e / (lambda1 - c);      // l.3
+    if (c_out) *c_out = c;
+    double sigma = sigma1;                        // l.5
+    if (m_max >= 1) {
+        alpha[1] = sigma1 / e;                    // l.4
+        beta[1] = 0.0;
+    }
+    for (int32_t k = 2; k <= m_max; ++k) {        // l.7
+        const double tau = 1.0 / (2.0 / sigma1 - sigma);   // l.8
+        alpha[k] = 2.0 * tau / e;                 // l.9
+        beta[k] = -tau * sigma;                   // l.9
+        sigma = tau;                              // l.11
+    }
+    return CHASE_OK;
+}
+
+int chase_filter_schedule(const int32_t *degrees, int64_t ncols, int32_t *offset) {
+    if (ncols < 0 || ncols > kMaxDim || (ncols > 0 && !degrees)) return CHASE_ERR_ARG;
+    int32_t prev = 0;
+    for (int64_t j = 0; j < ncols; ++j) {
+        if (degrees[j] < 0 || degrees[j] < prev) return CHASE_ERR_DEGREES;
+        prev = degrees[j];
+    }
+    const int32_t m_max = ncols ? degrees[ncols - 1] : 0;
+    if (offset) {
+        int64_t s = 0;
+        for (int32_t k = 1; k <= m_max; ++k) {    // l.12-14: drop columns whose degree is < k
+            while (s < ncols && degrees[s] < k) ++s;
+            offset[k] = (int32_t)s;
+        }
+    }
+    return m_max;
+}
+
+int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
+    if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0) return CHASE_ERR_ARG;
+    const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
+    if (force && force[0] == '1') return 0;
+    return dmma_supported(N, ncols, dtype) ? 1 : 0;
+}
+
+int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                    double a, double b, double lambda1, chase_dtype_t dtype,
+                    void *workspace, size_t workspace_bytes, void *stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t w = elem_bytes(dtype);
+    if (w == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return CHASE_ERR_ARG;
+    if (!H || (ncols > 0 && (!V || !degrees))) return CHASE_ERR_ARG;
+    if (!(std::isfinite(a) && std::isfinite(b) && std::isfinite(lambda1))) return CHASE_ERR_BOUNDS;
+    if (!(lambda1 < a && a < b)) return CHASE_ERR_BOUNDS;
+    const int m_max = chase_filter_schedule(degrees, ncols, nullptr);
+    if (m_max < 0) return m_max;
+    if (ncols == 0 || m_max == 0) return CHASE_OK;
+    if (!workspace || workspace_bytes < chase_filter_workspace_bytes(N, ncols, dtype))
+        return CHASE_ERR_WORKSPACE;
+    if (((uintptr_t)H | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
+
+    std::vector<int32_t> offset(m_max + 1);
+    std::vector<double> alpha(m_max + 1), beta(m_max + 1);
+    double c = 0.0;
+    chase_filter_schedule(degrees, ncols, offset.data());
+    int rc = chase_filter_scalars(a, b, lambda1, m_max, alpha.data(), beta.data(), &c);
+    if (rc != CHASE_OK) return rc;
+
+    // Two buffers, roles swapped after every step (Alg. 4 l.10; Listing 2):
+    // V_k lives in buf[k & 1]; step k reads buf[(k-1)&1] and overwrites V_{k-2} in buf[k&1]
+    // in place (V_{k-2} is an element-wise epilogue operand only, never a GEMM operand).
+    void *buf[2] = {V, workspace};
+    const size_t col_bytes = (size_t)N * w;
+
+    const bool use_dmma = chase_filter_kernel_path(N, ncols, dtype) == 1;
+    DmmaPlan plan;
+    if (use_dmma) {
+        cudaError_t e = dmma_plan_create(&plan, dtype, H, N, V, workspace, ncols);
+        if (e != cudaSuccess) return (int)e;
+    }
+
+    for (int k = 1; k <= m_max; ++k) {
+        const int64_t s = offset[k];
+        const int src = (k - 1) & 1;
+        cudaError_t e;
+        if (use_dmma) {
+            e = dmma_launch_step(&plan, src, s, alpha[k], beta[k], c, k > 1, stream);
+        } else {
+            StepArgs sa;
+            sa.H = H;
+            sa.X = (const char *)buf[src] + (size_t)s * col_bytes;
+            sa.Y = (char *)buf[src ^ 1] + (size_t)s * col_bytes;
+            sa.N = N;
+            sa.n = ncols - s;
+            sa.alpha = alpha[k];
+            sa.beta = beta[k];
+            sa.c = c;
+            sa.use_beta = k > 1;
+            e = launch_step_generic(dtype, sa, stream);
+        }
+        if (e != cudaSuccess) return (int)e;
+    }
+
+    // Result placement: V_{m_j} of an odd-degree column ended in the scratch
+    // buffer; copy each contiguous run of odd-degree columns back (none for Alg. 5's degrees).
+    for (int64_t j = 0; j < ncols;) {
+        if ((degrees[j] & 1) == 0) { ++j; continue; }
+        int64_t j1 = j;
+        while (j1 < ncols && (degrees[j1] & 1)) ++j1;
+        cudaError_t e = cudaMemcpyAsync((char *)V + (size_t)j * col_bytes,
+                                        (const char *)workspace + (size_t)j * col_bytes,
+                                        (size_t)(j1 - j) * col_bytes, cudaMemcpyDeviceToDevice, stream);
+        if (e != cudaSuccess) return (int)e;
+        j = j1;
+    }
+    return CHASE_OK;
+}
+
+int chase_filter(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                 double a, double b, double lambda1, chase_dtype_t dtype, void *stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (chase::elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return CHASE_ERR_ARG;
+    const int m_max = chase_filter_schedule(degrees, ncols, nullptr);
+    if (m_max < 0) return m_max;
+    if (ncols == 0 || m_max == 0) {
+        // still validate the remaining arguments the same way chase_filter_ws does
+        return chase_filter_ws(H, N, V, ncols, degrees, a, b, lambda1, dtype, nullptr, 0, stream_);
+    }
+    const size_t bytes = chase_filter_workspace_bytes(N, ncols, dtype);
+    void *ws = nullptr;
+    cudaError_t e = cudaMallocAsync(&ws, bytes, stream);
+    if (e != cudaSuccess) return (int)e;
+    int rc = chase_filter_ws(H, N, V, ncols, degrees, a, b, lambda1, dtype, ws, bytes, stream_);
+    e = cudaFreeAsync(ws, stream);
+    if (rc != CHASE_OK) return rc;
+    return e == cudaSuccess ? CHASE_OK : (int)e;
+}
+
+int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols,
+                      const int32_t *degrees, double a, double b, double lambda1,
+                      chase_dtype_t dtype, int device) {
+    const size_t w = chase::elem_bytes(dtype);
+    if (w == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return CHASE_ERR_ARG;
+    if (!H_host || (ncols > 0 && (!V_host || !degrees))) return CHASE_ERR_ARG;
+    if (!(std::isfinite(a) && std::isfinite(b) && std::isfinite(lambda1))) return CHASE_ERR_BOUNDS;
+    if (!(lambda1 < a && a < b)) return CHASE_ERR_BOUNDS;
+    const int m_max = chase_filter_schedule(degrees, ncols, nullptr);
+    if (m_max < 0) return m_max;
+    if (ncols == 0 || m_max == 0) return CHASE_OK;
+
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return (int)e;
+    const size_t hb = (size_t)N * (size_t)N * w, vb = (size_t)N * (size_t)ncols * w;
+    const size_t wb = chase_filter_workspace_bytes(N, ncols, dtype);
+    void *dH = nullptr, *dV = nullptr, *dW = nullptr;
+    cudaStream_t st = nullptr;
+    int rc = CHASE_OK;
+    auto fail = [&](cudaError_t err) { rc = (int)err; };
+    if ((e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking)) != cudaSuccess) return (int)e;
+    if ((e = cudaMalloc(&dH, hb)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK && (e = cudaMalloc(&dV, vb)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK && (e = cudaMalloc(&dW, wb)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK && (e = cudaMemcpyAsync(dV, V_host, vb, cudaMemcpyHostToDevice, st)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK && (e = cudaMemcpyAsync(dH, H_host, hb, cudaMemcpyHostToDevice, st)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK)
+        rc = chase_filter_ws(dH, N, dV, ncols, degrees, a, b, lambda1, dtype, dW, wb, (void *)st);
+    if (rc == CHASE_OK && (e = cudaMemcpyAsync(V_host, dV, vb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) fail(e);
+    e = cudaStreamSynchronize(st);
+    if (rc == CHASE_OK && e != cudaSuccess) fail(e);
+    cudaFree(dH);
+    cudaFree(dV);
+    cudaFree(dW);
+    cudaStreamDestroy(st);
+    return rc;
+}
+
+}  // extern "C"

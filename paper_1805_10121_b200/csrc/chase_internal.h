@@ -1,0 +1,48 @@
+// Internal declarations shared by the translation units of libchase_filter.so.
+// Not part of the public ABI (that is include/chase_filter.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "chase_filter.h"
+
+namespace chase {
+
+// One recurrence step (Alg. 4 line 4 / line 9) on `n` active columns:
+//   Y[:, j] <- alpha * (H X[:, j] - c X[:, j]) + beta * Y[:, j],   j = 0..n-1
+// X, Y are device pointers already offset to the first active column (ld = N).
+// use_beta == 0: Y is write-only (first step: the scratch buffer is uninitialised).
+struct StepArgs {
+    const void *H;
+    const void *X;
+    void *Y;
+    int64_t N;
+    int64_t n;
+    double alpha, beta, c;
+    int use_beta;
+};
+
+// Generic FMA kernels: any N, any n, all four dtypes.
+cudaError_t launch_step_generic(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
+
+// TMA + DMMA tensor kernels (CHASE_C128 with N % 8 == 0, CHASE_F64 with N % 16 == 0).
+// A plan holds the three tensor maps (H, and both vector buffers) of one chase_filter call.
+struct DmmaPlan {
+    alignas(64) unsigned char tmap_H[128];
+    alignas(64) unsigned char tmap_B[2][128];   // [0]: buffer V, [1]: buffer W
+    chase_dtype_t dtype;
+    int64_t N, ncols;
+    const void *H;
+    void *buf[2];
+};
+bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
+// Returns cudaSuccess, or an error (then the caller falls back to the generic kernels
+// only if the failure is "driver entry point unavailable"; anything else is reported).
+cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N,
+                             void *V, void *W, int64_t ncols);
+// Step reading buffer `src` (0/1) and writing buffer 1-src, active columns [s, ncols).
+cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
+                             double c, int use_beta, cudaStream_t stream);
+
+void count_launch();
+
+}  // namespace chase

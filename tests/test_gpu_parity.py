@@ -1,0 +1,159 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by element on
+the same seeded inputs.  Tolerances (north_star): rel. Frobenius <= 1e-12 for c128/f64,
+<= 1e-4 for c64/f32; also checked per column (a loose factor on the same bound) so that an
+error confined to one low-norm column cannot hide in the block norm."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1805_10121_b200 as pkg
+from paper_1805_10121_b200 import workloads as W
+from cheb_closed_form import p_m, rel_fro
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.complex128: 1e-12, torch.float64: 1e-12, torch.complex64: 1e-4, torch.float32: 1e-4}
+
+
+def _dev():
+    return torch.device("cuda:0")
+
+
+def to_device(x: torch.Tensor) -> torch.Tensor:
+    out = W.empty_colmajor(x.shape[0], x.shape[1], x.dtype, _dev())
+    out.copy_(x)
+    return out
+
+
+def run_gpu(w: W.Workload, degrees=None, use_ws=True, stream=None) -> np.ndarray:
+    H, V = to_device(w.H), to_device(w.V0)
+    deg = w.degrees if degrees is None else degrees
+    if use_ws:
+        ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=_dev())
+        ws.fill_(0xFF)          # NaN bit patterns: a read of uninitialised scratch would show
+        pkg.chase_filter_ws(H, V, deg, w.a, w.b, w.lambda1, ws, stream=stream)
+    else:
+        pkg.chase_filter(H, V, deg, w.a, w.b, w.lambda1, stream=stream)
+    torch.cuda.synchronize()
+    return V.cpu().numpy()
+
+
+def run_oracle(w: W.Workload, degrees=None) -> np.ndarray:
+    deg = w.degrees if degrees is None else degrees
+    return oracle.chase_filter(w.H.numpy(), w.V0.numpy(), np.asarray(deg), w.a, w.b, w.lambda1)
+
+
+def assert_parity(got, ref, dtype):
+    tol = TOL[dtype]
+    assert np.all(np.isfinite(got))
+    assert rel_fro(got, ref) <= tol
+    for j in range(ref.shape[1]):
+        nr = np.linalg.norm(ref[:, j])
+        if nr > 0:
+            assert np.linalg.norm(got[:, j] - ref[:, j]) / nr <= 10 * tol, j
+        else:
+            assert np.linalg.norm(got[:, j]) == 0
+
+
+def test_cfg1_full():
+    w = W.make_config(1)
+    got = run_gpu(w)
+    assert_parity(got, run_oracle(w), w.dtype)
+    # and against the paper's closed form (Eq. 5) directly
+    Q, lam = w.eigvecs.numpy(), w.eigvals.numpy().astype(np.float64)
+    coef = Q.conj().T @ w.V0.numpy()
+    ref = Q @ (p_m(10, lam, w.a, w.b, w.lambda1)[:, None] * coef)
+    assert rel_fro(got, ref) <= 1e-11
+
+
+@pytest.mark.parametrize("cfg,N,ncols", [
+    (2, 1024, 200),     # c128: several tiles + ragged column tail, sorted even degrees 10..30
+    (2, 520, 77),       # c128: N % 8 == 0 but not a tile multiple
+    (3, 1040, 150),     # f64: N % 16 == 0, uniform degree 20
+    (4, 776, 130),      # c128: degrees 8..36
+    (5, 768, 100),      # c64
+])
+def test_reduced_configs(cfg, N, ncols):
+    w = W.make_config(cfg, N=N, ncols=ncols)
+    assert_parity(run_gpu(w), run_oracle(w), w.dtype)
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64, torch.complex64, torch.complex128])
+@pytest.mark.parametrize("N,ncols", [(61, 5), (200, 33), (257, 1)])
+def test_generic_shapes_all_dtypes(dtype, N, ncols):
+    """Sizes no TMA path accepts (odd N): the generic FMA kernels, all four dtypes."""
+    w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
+    assert pkg.chase_filter_kernel_path(N, ncols, dtype) == 0
+    assert_parity(run_gpu(w), run_oracle(w), dtype)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.complex128])
+def test_odd_zero_and_one_degrees(dtype):
+    """Readings G5/G6: degree 0 untouched, degree 1 = first step only, odd degrees copied back."""
+    N, n = 272, 24
+    w = W.make_config(2, N=N, ncols=n, dtype=dtype)
+    deg = torch.tensor(sorted([0, 0, 1, 1, 2, 3, 3, 4, 5, 6, 7, 8, 8, 9, 10, 11, 12, 13, 14, 15, 15, 16, 17, 18]),
+                       dtype=torch.int32)
+    got = run_gpu(w, degrees=deg)
+    ref = run_oracle(w, degrees=deg.numpy())
+    assert_parity(got, ref, dtype)
+    assert np.array_equal(got[:, :2], w.V0.numpy()[:, :2])
+
+
+def test_internal_workspace_and_side_stream():
+    w = W.make_config(2, N=264, ncols=40)
+    ref = run_oracle(w)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        got = run_gpu(w, use_ws=False, stream=s)
+    assert_parity(got, ref, w.dtype)
+
+
+def test_launch_count_is_one_kernel_per_degree():
+    w = W.make_config(2, N=256, ncols=32)
+    H, V = to_device(w.H), to_device(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=_dev())
+    before = pkg.chase_filter_launch_count()
+    pkg.chase_filter_ws(H, V, w.degrees, w.a, w.b, w.lambda1, ws)
+    torch.cuda.synchronize()
+    assert pkg.chase_filter_launch_count() - before == int(w.degrees.max())
+
+
+def test_h_is_not_modified_and_inactive_columns_untouched():
+    w = W.make_config(2, N=256, ncols=32)
+    H, V = to_device(w.H), to_device(w.V0)
+    deg = w.degrees.clone()
+    deg[:5] = 0
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=_dev())
+    pkg.chase_filter_ws(H, V, deg, w.a, w.b, w.lambda1, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(H.cpu(), w.H)
+    assert torch.equal(V[:, :5].cpu(), w.V0[:, :5])
+
+
+def test_p9_uniform_vs_mixed_on_gpu():
+    w = W.make_config(4, N=512, ncols=64)
+    got = run_gpu(w)
+    deg = w.degrees.numpy()
+    for d in np.unique(deg)[:4]:
+        cols = np.nonzero(deg == d)[0]
+        sub = W.Workload("sub", w.H, W.as_colmajor(w.V0[:, cols]), torch.full((len(cols),), int(d), dtype=torch.int32),
+                         w.a, w.b, w.lambda1, w.dtype)
+        gsub = run_gpu(sub)
+        assert rel_fro(gsub, got[:, cols]) <= 1e-13
+
+
+def test_host_entry_point():
+    w = W.make_config(2, N=256, ncols=24)
+    V = w.V0.clone()
+    V = W.as_colmajor(V)
+    pkg.chase_filter_host(w.H, V, w.degrees, w.a, w.b, w.lambda1, device=0)
+    assert_parity(V.numpy(), run_oracle(w), w.dtype)
+
+
+def test_peak_probes_run():
+    dfma = pkg.chase_fp64_peak_probe(0, 2048)
+    dmma = pkg.chase_fp64_peak_probe(1, 2048)
+    print(f"FP64 peak probes: DFMA {dfma:.0f} GFLOP/s, DMMA {dmma:.0f} GFLOP/s")
+    assert dfma > 1000 and dmma > 1000

@@ -1,0 +1,125 @@
+"""CPU-only tests of the C-ABI library's host side: exported symbols, validation and error
+codes (all rejected before any CUDA call), the scalar recurrence and the active-suffix
+schedule (Alg. 4 l.2-5, 8, 11-14)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1805_10121_b200 as pkg
+from paper_1805_10121_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "chase_filter.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(chase_[a-z0-9_]+)\s*\(", header))
+    assert declared == set(binding.EXPORTS)
+    lib = ctypes.CDLL(pkg.lib_path())
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+def test_strerror_covers_codes():
+    for code in range(0, -7, -1):
+        assert pkg.chase_filter_strerror(code) != "unknown error"
+    assert pkg.chase_filter_strerror(-99) == "unknown error"
+
+
+def test_scalars_match_oracle_and_closed_form():
+    a, b, l1, m = -1.7, 2.05, -2.0, 36
+    alpha, beta, c = pkg.chase_filter_scalars(a, b, l1, m)
+    _, oalpha, obeta, oc, _ = oracle.chase_scalars(a, b, l1, m)
+    np.testing.assert_allclose(alpha[1:], oalpha[1:], rtol=1e-15)
+    np.testing.assert_allclose(beta[1:], obeta[1:], rtol=1e-15)
+    assert c == oc
+    assert beta[1] == 0.0
+
+
+@pytest.mark.parametrize("bounds", [(-1.0, -1.0, -2.0), (2.0, 1.0, -2.0), (-1.0, 2.0, -1.0),
+                                    (-1.0, 2.0, 0.0), (float("nan"), 2.0, -2.0), (-1.0, float("inf"), -2.0)])
+def test_scalars_reject_bad_bounds(bounds):
+    a, b, l1 = bounds
+    with pytest.raises(pkg.ChaseFilterError) as ei:
+        pkg.chase_filter_scalars(a, b, l1, 4)
+    assert ei.value.code == -2
+
+
+def test_schedule():
+    deg = [0, 0, 2, 2, 3, 6, 6]
+    m_max, off = pkg.chase_filter_schedule(deg)
+    assert m_max == 6
+    expect = [sum(1 for d in deg if d < k) for k in range(1, 7)]
+    assert list(off[1:]) == expect == [2, 2, 4, 5, 5, 5]
+    assert pkg.chase_filter_schedule([])[0] == 0
+    for bad in ([2, 1], [-1, 2], [4, 4, 2]):
+        with pytest.raises(pkg.ChaseFilterError) as ei:
+            pkg.chase_filter_schedule(bad)
+        assert ei.value.code == -3
+
+
+def _raw_ws(H=0x1000, N=64, V=0x2000, ncols=4, degrees=(2, 2, 4, 4), a=-1.0, b=2.0, l1=-2.0,
+            dtype=3, ws=0x3000, ws_bytes=1 << 20):
+    lib = pkg.load()
+    deg = np.asarray(degrees, dtype=np.int32)
+    return lib.chase_filter_ws(H, N, V, ncols, deg.ctypes.data if deg.size else None, a, b, l1, dtype,
+                               ws, ws_bytes, None)
+
+
+def test_validation_rejects_before_any_launch():
+    # fake (never dereferenced) device pointers: every call below must return before touching CUDA
+    assert _raw_ws(dtype=7) == -4
+    assert _raw_ws(N=0) == -1
+    assert _raw_ws(H=None) == -1
+    assert _raw_ws(V=None) == -1
+    assert _raw_ws(ncols=-1) == -1
+    assert _raw_ws(a=2.5) == -2
+    assert _raw_ws(l1=-0.5) == -2
+    assert _raw_ws(degrees=(4, 2, 4, 4)) == -3
+    assert _raw_ws(degrees=(-2, 2, 4, 4)) == -3
+    assert _raw_ws(ws=None) == -5
+    assert _raw_ws(ws_bytes=16) == -5
+    assert _raw_ws(H=0x1008) == -6
+    assert _raw_ws(ws=0x3004) == -6
+    # nothing to do: success without a launch, even with no workspace
+    before = pkg.chase_filter_launch_count()
+    assert _raw_ws(degrees=(0, 0, 0, 0), ws=None, ws_bytes=0) == 0
+    assert _raw_ws(ncols=0, degrees=(), V=None, ws=None, ws_bytes=0) == 0
+    assert pkg.chase_filter_launch_count() == before
+
+
+def test_workspace_bytes():
+    import torch
+    assert pkg.chase_filter_workspace_bytes(40000, 2000, torch.complex128) == 40000 * 2000 * 16
+    assert pkg.chase_filter_workspace_bytes(3, 1, torch.float32) == 256
+    assert pkg.load().chase_filter_workspace_bytes(10, 10, 9) == 0
+
+
+def test_binding_rejects_cpu_tensors_no_fallback():
+    import torch
+    from paper_1805_10121_b200 import workloads as W
+    w = W.make_config(2, N=32, ncols=4)
+    with pytest.raises(ValueError):
+        pkg.chase_filter(w.H, w.V0.clone(), w.degrees, w.a, w.b, w.lambda1)
+    with pytest.raises(ValueError):     # row-major input is a layout error, not silently transposed
+        pkg.chase_filter_host(torch.zeros(8, 8, dtype=torch.float64), torch.zeros(8, 2, dtype=torch.float64),
+                              [2, 2], -1.0, 2.0, -2.0)
+
+
+def test_product_does_not_import_oracle():
+    pkgdir = os.path.join(ROOT, "paper_1805_10121_b200")
+    for dirpath, _, files in os.walk(pkgdir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cuh")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src and "liboracle" not in src, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            src = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_1805_10121_b200" not in src and "from paper_1805_10121_b200" not in src, f
+            assert "#include \"chase" not in src, f
