@@ -1,7 +1,402 @@
-// placeholder until the TMA + DMMA kernel lands
+// TMA + FP64 tensor-core (DMMA) step kernel for complex128 and float64.
+//
+//   Y[:, j] <- alpha * (H X[:, j] - c X[:, j]) + beta * Y[:, j]     (Alg. 4 l.4 / l.9; Eq. 7)
+//
+// One kernel per degree step, one pass over H.  Structure:
+//   * 1 producer warp: one elected lane issues TMA (cp.async.bulk.tensor) loads of an H tile and
+//     an X tile per k-slab into a kStages-deep shared-memory ring, completion on mbarriers.
+//   * 8 consumer warps: fragments by LDS from the 128B-swizzled tiles, mma.sync m8n8k4 f64
+//     (SASS DMMA.8x8x4; sm_100a has no tcgen05 kind::f64), accumulators in registers,
+//     complex as 4 real products on interleaved data (one sign flip per H fragment).
+//   * fused epilogue in registers: -c X, alpha scaling, + beta Y (Y updated in place).
+//
+// Shared-memory tiles are rows of 128 bytes (8 complex / 16 real elements), TMA SWIZZLE_128B:
+//   A (H tile, M-major as stored): row index = mgroup * BK + k, the 128B hold 8 (16) consecutive
+//       matrix rows; loaded by ONE 3-D TMA box {16 doubles, BK, BM/rows_per_128B} from the view
+//       (m_in_group, k, m_group) of the column-major H.
+//   B (X tile, K-major as stored): row index = kgroup * BN + n, the 128B hold 8 (16) consecutive k.
+// The k index each MMA lane slot consumes is a free permutation; it is chosen so that every
+// fragment load is bank-conflict free under the swizzle (complex: k = 8q + 2t + a; real:
+// k = {0,3,12,15}[t] ^ {0,1,4,5}[a]), identically for A and B.
+#include <cuda.h>
+
+#include <mutex>
+
 #include "chase_internal.h"
+
 namespace chase {
-bool dmma_supported(int64_t, int64_t, chase_dtype_t) { return false; }
-cudaError_t dmma_plan_create(DmmaPlan *, chase_dtype_t, const void *, int64_t, void *, void *, int64_t) { return cudaErrorNotSupported; }
-cudaError_t dmma_launch_step(const DmmaPlan *, int, int64_t, double, double, double, int, cudaStream_t) { return cudaErrorNotSupported; }
+namespace {
+
+constexpr int kConsumerWarps = 8;
+constexpr int kThreads = (kConsumerWarps + 4) * 32;   // 2 consumer warpgroups + 1 producer warpgroup
+constexpr int BK = 16;   // k elements per pipeline stage
+
+template <bool CPLX>
+struct Cfg;
+template <>
+struct Cfg<true> {   // complex128: CTA tile 128 x 64, warp tile 32 x 32 (4 x 2 warps)
+    static constexpr int BM = 128, BN = 64, WM = 32, WN = 32, WARPS_M = 4;
+    static constexpr int ROWS128 = 8;       // matrix rows (or k) per 128-byte smem row
+    static constexpr int ESZ = 16;
+    static constexpr int STAGES = 4;
+};
+template <>
+struct Cfg<false> {  // float64: CTA tile 128 x 128, warp tile 64 x 32 (2 x 4 warps)
+    static constexpr int BM = 128, BN = 128, WM = 64, WN = 32, WARPS_M = 2;
+    static constexpr int ROWS128 = 16;
+    static constexpr int ESZ = 8;
+    static constexpr int STAGES = 6;
+};
+
+template <bool CPLX>
+struct Smem {
+    static constexpr int A_BYTES = Cfg<CPLX>::BM * BK * Cfg<CPLX>::ESZ;
+    static constexpr int B_BYTES = Cfg<CPLX>::BN * BK * Cfg<CPLX>::ESZ;
+    static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+    static constexpr int TOTAL = Cfg<CPLX>::STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
+};
+
+// ---------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
 }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// ---------------------------------------------------------------- the kernel
+struct StepParams {
+    const double *X;     // source iterate V_k, first ACTIVE column (ld = N elements)
+    double *Y;           // destination (holds V_{k-1}, becomes V_{k+1}), first active column
+    int64_t N;           // matrix order
+    int n;               // active columns
+    int col0;            // first active column in the full buffer (TMA coordinate offset)
+    int tiles_m, tiles_n;
+    double alpha, beta, c;
+    int use_beta;
+};
+
+// Grouped rasterisation: consecutive CTAs cover kGroupN column tiles x a run of row tiles, so the
+// CTAs resident at one time share both H row panels and X column panels in L2.
+constexpr int kGroupN = 8;
+__device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
+    const int per_group = kGroupN * tiles_m;
+    const int grp = t / per_group;
+    const int first_n = grp * kGroupN;
+    const int gn = min(kGroupN, tiles_n - first_n);
+    const int r = t - grp * per_group;
+    tm = r / gn;
+    tn = first_n + r % gn;
+}
+
+template <bool CPLX>
+__global__ void __launch_bounds__(kThreads, 1)
+step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
+                 const StepParams p) {
+    using C = Cfg<CPLX>;
+    using S = Smem<CPLX>;
+    constexpr int BM = C::BM, BN = C::BN, STAGES = C::STAGES;
+    constexpr int MB = C::WM / 8, NB = C::WN / 8;   // 8x8 MMA blocks per warp tile
+
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    // 1024B alignment for SWIZZLE_128B; offset arithmetic keeps the pointer in the shared space
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_base + STAGES * S::STAGE_BYTES;   // full[STAGES], empty[STAGES]
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int tile_m, tile_n;
+    tile_coords(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
+    const int m0 = tile_m * BM, n0 = tile_n * BN;
+    const int KT = (int)((p.N + BK - 1) / BK);
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_base + 8 * s, 1);                          // full: producer's expect_tx arrive
+            mbar_init(bar_base + 8 * (STAGES + s), kConsumerWarps);  // empty: one arrive per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= kConsumerWarps) {
+        // ------------------------------------------------------------ producer warpgroup
+        // gives its registers to the consumers (setmaxnreg is per warpgroup); one lane issues TMA
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == kConsumerWarps && lane == 0) {
+            for (int kt = 0; kt < KT; ++kt) {
+                const int s = kt % STAGES;
+                const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
+                if (kt >= STAGES) mbar_wait(empty, ((kt / STAGES) - 1) & 1);
+                const uint32_t sa = smem_base + s * S::STAGE_BYTES, sb = sa + S::A_BYTES;
+                mbar_expect_tx(full, S::STAGE_BYTES);
+                const int k0 = kt * BK;
+                // A: view (16 doubles, k, m_group); one box {16, BK, BM / ROWS128}
+                tma_load_3d(sa, &tmapA, full, 0, k0, m0 / C::ROWS128);
+                // B: (doubles along k, column); boxes {16 doubles, BN}
+                if (CPLX) {
+                    tma_load_2d(sb, &tmapB, full, 2 * k0, p.col0 + n0);
+                    tma_load_2d(sb + BN * 128, &tmapB, full, 2 * k0 + 16, p.col0 + n0);
+                } else {
+                    tma_load_2d(sb, &tmapB, full, k0, p.col0 + n0);
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------- consumer warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    const int g = lane >> 2, t = lane & 3;
+    const int wm = warp % C::WARPS_M, wn = warp / C::WARPS_M;
+
+    double acc[CPLX ? 2 : 1][MB][NB][2];
+#pragma unroll
+    for (int q = 0; q < (CPLX ? 2 : 1); ++q)
+#pragma unroll
+        for (int i = 0; i < MB; ++i)
+#pragma unroll
+            for (int j = 0; j < NB; ++j) acc[q][i][j][0] = acc[q][i][j][1] = 0.0;
+
+    for (int kt = 0; kt < KT; ++kt) {
+        const int s = kt % STAGES;
+        mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
+        const unsigned char *sa = smem + s * S::STAGE_BYTES;
+        const unsigned char *sb = sa + S::A_BYTES;
+
+        if (CPLX) {
+            // 128B row = 8 complex.  A row index = mg*BK + k (mg = 8-row group), chunk = m ^ (k&7).
+            //                        B row index = kg*BN + n (kg = 8-k group),  chunk = (k&7) ^ (n&7).
+#pragma unroll
+            for (int kq = 0; kq < BK / 8; ++kq) {
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    const int k7 = 2 * t + a;            // k & 7 of this lane's slot
+                    const int k = kq * 8 + k7;
+                    double ar[MB], ai[MB], nai[MB];
+#pragma unroll
+                    for (int i = 0; i < MB; ++i) {
+                        const int mg = wm * (C::WM / 8) + i;
+                        const double2 v = *reinterpret_cast<const double2 *>(
+                            sa + (mg * BK + k) * 128 + ((g ^ k7) << 4));
+                        ar[i] = v.x; ai[i] = v.y; nai[i] = -v.y;
+                    }
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        const int n = wn * C::WN + j * 8 + g;
+                        const double2 b = *reinterpret_cast<const double2 *>(
+                            sb + (kq * BN + n) * 128 + ((k7 ^ g) << 4));
+#pragma unroll
+                        for (int i = 0; i < MB; ++i) {
+                            dmma884(acc[0][i][j][0], acc[0][i][j][1], ar[i], b.x);    // Cr += Ar Br
+                            dmma884(acc[0][i][j][0], acc[0][i][j][1], nai[i], b.y);   // Cr -= Ai Bi
+                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ar[i], b.y);    // Ci += Ar Bi
+                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ai[i], b.x);    // Ci += Ai Br
+                        }
+                    }
+                }
+            }
+        } else {
+            // 128B row = 16 doubles.  A row index = mg*BK + k (mg = 16-row group), chunk = (m>>1) ^ (k&7);
+            //                         B row index = n (BK = 16 = one k group),    chunk = (k>>1) ^ (n&7).
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                const int k = ((t == 0) ? 0 : (t == 1) ? 3 : (t == 2) ? 12 : 15) ^ ((a & 1) | ((a & 2) << 1));
+                double af[MB];
+#pragma unroll
+                for (int i = 0; i < MB; ++i) {
+                    const int mg = wm * (C::WM / 16) + (i >> 1);
+                    const int ml = g + 8 * (i & 1);
+                    af[i] = *reinterpret_cast<const double *>(
+                        sa + (mg * BK + k) * 128 + (((ml >> 1) ^ (k & 7)) << 4) + ((ml & 1) << 3));
+                }
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    const int n = wn * C::WN + j * 8 + g;
+                    const double b = *reinterpret_cast<const double *>(
+                        sb + n * 128 + ((((k >> 1) & 7) ^ g) << 4) + ((k & 1) << 3));
+#pragma unroll
+                    for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+    }
+
+    // ---------------------------------------------------------------- fused epilogue
+    // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
+    const double alpha = p.alpha, beta = p.beta, c = p.c;
+    constexpr int NC = CPLX ? 2 : 1;
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int col = n0 + wn * C::WN + j * 8 + 2 * t + e;
+            if (col >= p.n) continue;
+#pragma unroll
+            for (int i = 0; i < MB; ++i) {
+                int row;
+                if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
+                else row = m0 + wm * C::WM + (i >> 1) * 16 + (i & 1) * 8 + g;
+                if (row >= p.N) continue;
+                const int64_t off = ((int64_t)col * p.N + row) * NC;
+                if (CPLX) {
+                    const double2 x = *reinterpret_cast<const double2 *>(p.X + off);
+                    double2 y;
+                    y.x = alpha * (acc[0][i][j][e] - c * x.x);
+                    y.y = alpha * (acc[NC - 1][i][j][e] - c * x.y);
+                    if (p.use_beta) {
+                        const double2 o = *reinterpret_cast<const double2 *>(p.Y + off);
+                        y.x = fma(beta, o.x, y.x);
+                        y.y = fma(beta, o.y, y.y);
+                    }
+                    *reinterpret_cast<double2 *>(p.Y + off) = y;
+                } else {
+                    double y = alpha * (acc[0][i][j][e] - c * p.X[off]);
+                    if (p.use_beta) y = fma(beta, p.Y[off], y);
+                    p.Y[off] = y;
+                }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------- host side
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                   CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    });
+    return fn;
+}
+
+template <bool CPLX>
+cudaError_t encode_maps(DmmaPlan *plan) {
+    using C = Cfg<CPLX>;
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return cudaErrorNotSupported;
+    const cuuint64_t N = (cuuint64_t)plan->N;
+    {   // A: H viewed as (16 doubles, k, m_group)
+        cuuint64_t dims[3] = {16, N, N / C::ROWS128};
+        cuuint64_t strides[2] = {N * C::ESZ, 128};
+        cuuint32_t box[3] = {16, BK, (cuuint32_t)(C::BM / C::ROWS128)};
+        cuuint32_t estr[3] = {1, 1, 1};
+        CUresult r = enc((CUtensorMap *)plan->tmap_H, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)plan->H, dims,
+                         strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    for (int b = 0; b < 2; ++b) {   // B: a vector buffer viewed as (doubles along k, column)
+        cuuint64_t dims[2] = {N * (CPLX ? 2 : 1), (cuuint64_t)plan->ncols};
+        cuuint64_t strides[1] = {N * C::ESZ};
+        cuuint32_t box[2] = {16, (cuuint32_t)C::BN};
+        cuuint32_t estr[2] = {1, 1};
+        CUresult r = enc((CUtensorMap *)plan->tmap_B[b], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, plan->buf[b], dims,
+                         strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    }
+    return cudaSuccess;
+}
+
+template <bool CPLX>
+cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
+                   cudaStream_t stream) {
+    using C = Cfg<CPLX>;
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(step_dmma_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        Smem<CPLX>::TOTAL);
+    });
+    if (attr_err != cudaSuccess) return attr_err;
+    const int64_t n = plan->ncols - s;
+    if (n <= 0) return cudaSuccess;
+    StepParams p;
+    const size_t col_doubles = (size_t)plan->N * (CPLX ? 2 : 1);
+    p.X = (const double *)plan->buf[src] + (size_t)s * col_doubles;
+    p.Y = (double *)plan->buf[src ^ 1] + (size_t)s * col_doubles;
+    p.N = plan->N;
+    p.n = (int)n;
+    p.col0 = (int)s;
+    p.tiles_m = (int)((plan->N + C::BM - 1) / C::BM);
+    p.tiles_n = (int)((n + C::BN - 1) / C::BN);
+    p.alpha = alpha;
+    p.beta = beta;
+    p.c = c;
+    p.use_beta = use_beta;
+    const CUtensorMap *mA = (const CUtensorMap *)plan->tmap_H;
+    const CUtensorMap *mB = (const CUtensorMap *)plan->tmap_B[src];
+    step_dmma_kernel<CPLX><<<(unsigned)(p.tiles_m * p.tiles_n), kThreads, Smem<CPLX>::TOTAL, stream>>>(*mA, *mB, p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
+    if (ncols < 1 || N < 16 || N > (1 << 28) || ncols > (1 << 28)) return false;
+    if (dtype == CHASE_C128) return N % 8 == 0;
+    if (dtype == CHASE_F64) return N % 16 == 0;
+    return false;
+}
+
+cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V, void *W,
+                             int64_t ncols) {
+    plan->dtype = dtype;
+    plan->N = N;
+    plan->ncols = ncols;
+    plan->H = H;
+    plan->buf[0] = V;
+    plan->buf[1] = W;
+    return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);
+}
+
+cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c,
+                             int use_beta, cudaStream_t stream) {
+    return plan->dtype == CHASE_C128 ? launch<true>(plan, src, s, alpha, beta, c, use_beta, stream)
+                                     : launch<false>(plan, src, s, alpha, beta, c, use_beta, stream);
+}
+
+}  // namespace chase

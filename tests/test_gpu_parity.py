@@ -80,7 +80,7 @@ def test_reduced_configs(cfg, N, ncols):
 
 
 @pytest.mark.parametrize("dtype", [torch.float32, torch.float64, torch.complex64, torch.complex128])
-@pytest.mark.parametrize("N,ncols", [(61, 5), (200, 33), (257, 1)])
+@pytest.mark.parametrize("N,ncols", [(61, 5), (203, 33), (257, 1)])
 def test_generic_shapes_all_dtypes(dtype, N, ncols):
     """Sizes no TMA path accepts (odd N): the generic FMA kernels, all four dtypes."""
     w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
