@@ -1,0 +1,393 @@
+#!/usr/bin/env python
+"""bench.py -- Chebyshev-filter throughput on B200 (BASELINE.json metric).
+
+A "step" is one chase_filter_ws call (the whole hot path: host scalars + schedule, one fused
+TMA/DMMA step kernel per degree) on the workload BASELINE.json quotes the metric on:
+cfg 4 = N=40000 complex128 GUE, V0 40000x2000, sorted even degrees 8..36 (synthetic, seeded).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 4]
+
+Prints ONE JSON line (rank 0).  `value` = filter GFLOP/s = 8 N^2 sum(deg) / t (complex; 2 N^2
+sum(deg) real), whole job, inputs resident in HBM.  `e2e` = same metric through
+chase_filter_host (HOST buffers, H2D/D2H inside the timed region).  `roofline` = achieved
+TFLOP/s of the step kernel vs the FP64 peak.  `cpu_baseline` = the oracle,
+as it stands, on the host cores on a bounded sample.  --impl reference times the oracle.
+Multi-GPU (--gpus N under torchrun): independent column batches per rank, H replicated, no
+data-path collective; scaling = weak.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_1805_10121_b200 import workloads as W
+
+METRIC = "chebyshev_filter_gflops"
+UNIT = "GFLOP/s"
+# FP64 peak: 148 SMs x 128 FP64 flop/clk/SM x 1.965 GHz (clocks.max.sm).
+# The DMMA.8x8x4 and DFMA pipes have the same rate; a register-only probe run live below
+# (chase_fp64_peak_probe) measures it on this very GPU.
+FP64_FLOP_PER_CLK_SM = 128
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 = metric config")
+    ap.add_argument("--N", type=int, default=None, help="override N (debug only; prints config.reduced)")
+    ap.add_argument("--ncols", type=int, default=None)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sample-cols", type=int, default=16)
+    ap.add_argument("--sample-degree", type=int, default=8)
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.thread.join(timeout=2)
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(smax), "power_w_max": max(power),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_setup(ngpus: int):
+    """(rank, world, local_rank); initialises NCCL only when launched under torchrun."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(local)
+        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local))
+    return rank, world, local
+
+
+def barrier(world: int):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def max_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(x: float, world: int) -> float:
+    if world == 1:
+        return x
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device="cuda")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# ----------------------------------------------------------------------------------------------
+# workload
+# ----------------------------------------------------------------------------------------------
+def build_workload(args, device, rank: int) -> W.Workload:
+    w = W.make_config(args.config, device=device, N=args.N, ncols=args.ncols)
+    if rank > 0:   # independent batch per rank: same H (replicated), different seeded V0
+        seed = W.BASE_SEED + 1000 * args.config + 1 + 10 * rank
+        w.V0 = W.gaussian_colmajor(w.N, w.ncols, w.dtype, seed, device)
+    return w
+
+
+def workload_config(args, w: W.Workload, world: int) -> dict:
+    cfg = {
+        "workload": f"BASELINE.json configs[{args.config - 1}] (cfg {args.config}): N={w.N} "
+                    f"{W.DTYPE_NAMES[w.dtype]} Hermitian, V0 {w.N}x{w.ncols}, degrees "
+                    f"{int(w.degrees.min())}..{int(w.degrees.max())} sorted, sum_deg={w.sum_deg}",
+        "N": w.N, "ncols_per_gpu": w.ncols, "sum_deg_per_gpu": w.sum_deg,
+        "a": w.a, "b": w.b, "lambda1": w.lambda1,
+        "l2": (f"inputs exceed L2 (H = {w.H.numel() * w.H.element_size() / 1e9:.1f} GB > 126 MB); no flush needed"
+               if w.H.numel() * w.H.element_size() >= (512 << 20) else "L2 flushed (512 MB write) between iterations"),
+        "parallelism": "single GPU" if world == 1 else f"{world} independent column batches, H replicated, no collective",
+    }
+    if args.N is not None or args.ncols is not None:
+        cfg["reduced"] = True
+    return cfg
+
+
+def sample_columns(w: W.Workload, k: int):
+    k = min(k, w.ncols)
+    return [int(round(i * (w.ncols - 1) / max(k - 1, 1))) for i in range(k)] if k > 1 else [0]
+
+
+def host_colmajor_numpy(x: torch.Tensor) -> np.ndarray:
+    """Device (or host) column-major tensor -> Fortran-ordered numpy array, one copy."""
+    return x.t().cpu().t().numpy()
+
+
+def oracle_sample_run(Hn: np.ndarray, Vn: np.ndarray, degree: int, w):
+    """Times the oracle, as it stands, on `Vn` (column sample) with a uniform truncated degree.
+    Returns (seconds, flops, result)."""
+    import oracle
+    deg = np.full(Vn.shape[1], degree, dtype=np.int32)
+    f = 8.0 if np.iscomplexobj(Hn) else 2.0
+    t0 = time.perf_counter()
+    out = oracle.chase_filter(Hn, Vn, deg, w.a, w.b, w.lambda1)
+    dt = time.perf_counter() - t0
+    return dt, f * float(Hn.shape[0]) ** 2 * Vn.shape[1] * degree, out
+
+
+# ----------------------------------------------------------------------------------------------
+# --impl reference : the oracle on the host cores (tier framing (4))
+# ----------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    device = torch.device("cuda:0") if torch.cuda.is_available() else torch.device("cpu")
+    w = build_workload(args, device, 0)    # the GPU, if present, only generates the inputs
+    cols = sample_columns(w, args.sample_cols)
+    Hn = host_colmajor_numpy(w.H)
+    Vn = np.asfortranarray(host_colmajor_numpy(w.V0)[:, cols])
+    cfg = workload_config(args, w, 1)
+    N, ncols = w.N, w.ncols
+    w.H = None
+    w.V0 = None
+    if device.type == "cuda":
+        torch.cuda.empty_cache()
+    for _ in range(args.warmup):
+        oracle_sample_run(Hn, Vn, args.sample_degree, w)
+    times, flops = [], 0.0
+    for _ in range(args.steps):
+        dt, fl, _ = oracle_sample_run(Hn, Vn, args.sample_degree, w)
+        times.append(dt)
+        flops = fl
+    total = sum(times)
+    value = flops * args.steps / total * 1e-9
+    sample = (f"{len(cols)} of {ncols} columns (evenly spaced), full {N}x{N} H, degree truncated to "
+              f"{args.sample_degree}; one step = one oracle call on that sample")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": cfg,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ----------------------------------------------------------------------------------------------
+# our arm
+# ----------------------------------------------------------------------------------------------
+def run_ours(args):
+    import paper_1805_10121_b200 as pkg
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    pkg.load()
+    rank, world, local = dist_setup(args.gpus)
+    device = torch.device("cuda", local)
+    torch.cuda.set_device(device)
+
+    w = build_workload(args, device, rank)
+    N, n, dtype = w.N, w.ncols, w.dtype
+    V = W.empty_colmajor(N, n, dtype, device)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(N, n, dtype), dtype=torch.uint8, device=device)
+    stream = torch.cuda.Stream(device)
+    flops_step = w.flops()
+    h_bytes = w.H.numel() * w.H.element_size()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=device) if h_bytes < (512 << 20) else None
+
+    def one_step(timed: bool):
+        V.copy_(w.V0)                       # restore V0 outside the timed region
+        if flush is not None:
+            flush.zero_()                   # inputs fit in L2: flush it between iterations
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            pkg.chase_filter_ws(w.H, V, w.degrees, w.a, w.b, w.lambda1, ws, stream=stream)
+            e1.record(stream)
+        torch.cuda.current_stream().wait_stream(stream)
+        return (e0, e1) if timed else None
+
+    for _ in range(args.warmup):
+        one_step(False)
+    barrier(world)
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = pkg.chase_filter_launch_count()
+    barrier(world)
+    t_wall0 = time.perf_counter()
+    events = [one_step(True) for _ in range(args.steps)]
+    barrier(world)
+    t_wall = time.perf_counter() - t_wall0
+    launches = pkg.chase_filter_launch_count() - launches0
+    clocks = sampler.stop() if rank == 0 else None
+
+    dev_s = sum(e0.elapsed_time(e1) for e0, e1 in events) * 1e-3     # device time of the K filter calls
+    dev_s = max_over_ranks(dev_s, world)
+    total_flops = sum_over_ranks(flops_step * args.steps, world)
+    value = total_flops / dev_s * 1e-9
+
+    # ---- roofline of the step kernel (all launches of a step are the same kernel) --------------
+    sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+    sms = torch.cuda.get_device_properties(device).multi_processor_count
+    peak_nominal = sms * FP64_FLOP_PER_CLK_SM * sm_max_mhz * 1e6 * 1e-12        # TFLOP/s
+    probe_dmma = pkg.chase_fp64_peak_probe(1, 1 << 16) * 1e-3
+    probe_dfma = pkg.chase_fp64_peak_probe(0, 1 << 16) * 1e-3
+    achieved = flops_step * args.steps / (sum(e0.elapsed_time(e1) for e0, e1 in events) * 1e-3) * 1e-12
+    kernel_path = pkg.chase_filter_kernel_path(N, n, dtype)
+    is_f64 = dtype in (torch.complex128, torch.float64)
+    if not is_f64:
+        peak_nominal *= 2.0       # FP32 FMA pipe: 256 flop/clk/SM
+    roofline = {
+        "bound": "tensor" if kernel_path == 1 else "alu",
+        "kernel": "step_dmma_kernel" if kernel_path == 1 else "step_generic_kernel",
+        "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
+        "traffic": None,
+        "peak_source": f"{sms} SMs x {FP64_FLOP_PER_CLK_SM * (1 if is_f64 else 2)} flop/clk/SM x clocks.max.sm "
+                       f"{sm_max_mhz:.0f} MHz (DESIGN.md 'Peak'); MEASURED_PEAKS.json has no FP64 entry",
+        "peak_probe_dmma_tflops": probe_dmma, "peak_probe_dfma_tflops": probe_dfma,
+        "frac_of_probe_dmma": achieved / probe_dmma if is_f64 else None,
+        "frac_of_nvidia_quoted_40tf": achieved / 40.0 if is_f64 else None,
+        "algorithmic_flops_per_step": flops_step, "launches_per_step": launches // max(args.steps, 1),
+    }
+
+    # ---- sampled parity + cpu_baseline (rank 0, N = 1): the oracle on a bounded sample ---------
+    cpu_baseline, parity = None, None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        cols = sample_columns(w, args.sample_cols)
+        Hn = host_colmajor_numpy(w.H)
+        Vs = W.as_colmajor(w.V0[:, cols])
+        dt, fl, ref = oracle_sample_run(Hn, host_colmajor_numpy(Vs), args.sample_degree, w)
+        del Hn
+        wss = torch.empty(pkg.chase_filter_workspace_bytes(N, len(cols), dtype), dtype=torch.uint8, device=device)
+        pkg.chase_filter_ws(w.H, Vs, [args.sample_degree] * len(cols), w.a, w.b, w.lambda1, wss)
+        torch.cuda.synchronize()
+        got = host_colmajor_numpy(Vs)
+        sample = (f"{len(cols)} of {n} columns (evenly spaced), full {N}x{N} H, degree truncated to "
+                  f"{args.sample_degree}")
+        cpu_baseline = {"value": fl / dt * 1e-9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                        "sample": sample, "seconds": dt}
+        parity = {"rel_fro_vs_oracle": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)), "sample": sample}
+
+    # ---- e2e: HOST buffers through chase_filter_host (H2D + filter + D2H inside the timed call) --
+    e2e = None
+    if not args.no_e2e:
+        Hh = torch.empty((N, N), dtype=dtype, pin_memory=True)
+        Hh.copy_(w.H.t())
+        Vh = torch.empty((n, N), dtype=dtype, pin_memory=True)
+        Vh.copy_(w.V0.t())
+        torch.cuda.synchronize()
+        barrier(world)
+        t0 = time.perf_counter()
+        pkg.chase_filter_host(Hh.t(), Vh.t(), w.degrees, w.a, w.b, w.lambda1, device=local)
+        barrier(world)
+        e2e_s = max_over_ranks(time.perf_counter() - t0, world)
+        h2d = Hh.numel() * Hh.element_size() + Vh.numel() * Vh.element_size()
+        d2h = Vh.numel() * Vh.element_size()
+        e2e = {"value": sum_over_ranks(flops_step, world) / e2e_s * 1e-9, "unit": UNIT,
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": 1, "seconds": e2e_s,
+               "api": "chase_filter_host (pinned host H, V; cudaMalloc + H2D + filter + D2H + free inside)"}
+        del Hh, Vh
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dev_s / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": {torch.complex128: "c128 (f64 arithmetic)",
+                                                               torch.float64: "f64", torch.complex64: "c64 (f32 arithmetic)",
+                                                               torch.float32: "f32"}[dtype],
+            "data": "synthetic", "config": workload_config(args, w, world), "clocks": clocks,
+            "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "parity": parity, "wall_s_timed_region": t_wall,
+            "fraction_of_fp64_peak": roofline["frac"] if is_f64 else None,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
