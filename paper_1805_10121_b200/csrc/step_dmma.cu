@@ -29,7 +29,6 @@ namespace {
 
 constexpr int kConsumerWarps = 8;
 constexpr int kThreads = (kConsumerWarps + 4) * 32;   // 2 consumer warpgroups + 1 producer warpgroup
-constexpr int BK = 16;   // k elements per pipeline stage
 
 template <bool CPLX>
 struct Cfg;
@@ -38,20 +37,24 @@ struct Cfg<true> {   // complex128: CTA tile 128 x 64, warp tile 32 x 32 (4 x 2 
     static constexpr int BM = 128, BN = 64, WM = 32, WN = 32, WARPS_M = 4;
     static constexpr int ROWS128 = 8;       // matrix rows (or k) per 128-byte smem row
     static constexpr int ESZ = 16;
+    static constexpr int BK = 16;           // k elements per pipeline stage (48 KB / stage)
     static constexpr int STAGES = 4;
+    static constexpr int GROUP_N = 16;      // raster group: 16 column tiles x ~9 row tiles per wave
 };
 template <>
 struct Cfg<false> {  // float64: CTA tile 128 x 128, warp tile 64 x 32 (2 x 4 warps)
     static constexpr int BM = 128, BN = 128, WM = 64, WN = 32, WARPS_M = 2;
     static constexpr int ROWS128 = 16;
     static constexpr int ESZ = 8;
-    static constexpr int STAGES = 6;
+    static constexpr int BK = 32;           // 64 KB / stage: same DMMA count per stage as complex
+    static constexpr int STAGES = 3;
+    static constexpr int GROUP_N = 12;
 };
 
 template <bool CPLX>
 struct Smem {
-    static constexpr int A_BYTES = Cfg<CPLX>::BM * BK * Cfg<CPLX>::ESZ;
-    static constexpr int B_BYTES = Cfg<CPLX>::BN * BK * Cfg<CPLX>::ESZ;
+    static constexpr int A_BYTES = Cfg<CPLX>::BM * Cfg<CPLX>::BK * Cfg<CPLX>::ESZ;
+    static constexpr int B_BYTES = Cfg<CPLX>::BN * Cfg<CPLX>::BK * Cfg<CPLX>::ESZ;
     static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
     static constexpr int TOTAL = Cfg<CPLX>::STAGES * STAGE_BYTES + 1024 /*align slack*/ + 256 /*barriers*/;
 };
@@ -107,8 +110,10 @@ struct StepParams {
 };
 
 // Grouped rasterisation: consecutive CTAs cover kGroupN column tiles x a run of row tiles, so the
-// CTAs resident at one time share both H row panels and X column panels in L2.
-constexpr int kGroupN = 8;
+// CTAs resident at one time share both H row panels and X column panels in L2.  kGroupN is chosen
+// so that a wave of 148 CTAs is roughly square in BYTES (rows*BM ~ cols*BN), which minimises the
+// DRAM traffic of 148 register-resident output tiles.
+template <int kGroupN>
 __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
     const int per_group = kGroupN * tiles_m;
     const int grp = t / per_group;
@@ -125,7 +130,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                  const StepParams p) {
     using C = Cfg<CPLX>;
     using S = Smem<CPLX>;
-    constexpr int BM = C::BM, BN = C::BN, STAGES = C::STAGES;
+    constexpr int BM = C::BM, BN = C::BN, BK = C::BK, STAGES = C::STAGES;
     constexpr int MB = C::WM / 8, NB = C::WN / 8;   // 8x8 MMA blocks per warp tile
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -136,7 +141,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int tile_m, tile_n;
-    tile_coords(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
+    tile_coords<C::GROUP_N>(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
     const int m0 = tile_m * BM, n0 = tile_n * BN;
     const int KT = (int)((p.N + BK - 1) / BK);
 
@@ -168,7 +173,9 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                     tma_load_2d(sb, &tmapB, full, 2 * k0, p.col0 + n0);
                     tma_load_2d(sb + BN * 128, &tmapB, full, 2 * k0 + 16, p.col0 + n0);
                 } else {
-                    tma_load_2d(sb, &tmapB, full, k0, p.col0 + n0);
+#pragma unroll
+                    for (int kq = 0; kq < BK / 16; ++kq)
+                        tma_load_2d(sb + kq * BN * 128, &tmapB, full, k0 + 16 * kq, p.col0 + n0);
                 }
             }
         }
@@ -187,6 +194,16 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
         for (int i = 0; i < MB; ++i)
 #pragma unroll
             for (int j = 0; j < NB; ++j) acc[q][i][j][0] = acc[q][i][j][1] = 0.0;
+
+    // float64: lane-dependent byte offsets of the fragment loads, hoisted out of the k loop.
+    // MMA a of a 16-k group consumes, in lane slot t, k = {0,3,12,15}[t] ^ {0,1,4,5}[a] (conflict-free).
+    int real_a_off[4], real_b_off[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        const int kl = (3 * (t & 1) + 12 * (t >> 1)) ^ ((a & 1) | ((a & 2) << 1));
+        real_a_off[a] = kl * 128 + (((g >> 1) ^ (kl & 7)) << 4) + ((g & 1) << 3);     // row ml = g; ml = g+8: ^ 64
+        real_b_off[a] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4) + ((kl & 1) << 3);
+    }
 
     for (int kt = 0; kt < KT; ++kt) {
         const int s = kt % STAGES;
@@ -228,25 +245,25 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
             }
         } else {
             // 128B row = 16 doubles.  A row index = mg*BK + k (mg = 16-row group), chunk = (m>>1) ^ (k&7);
-            //                         B row index = n (BK = 16 = one k group),    chunk = (k>>1) ^ (n&7).
+            //                         B row index = kg*BN + n (kg = 16-k group),   chunk = (k>>1) ^ (n&7).
 #pragma unroll
-            for (int a = 0; a < 4; ++a) {
-                const int k = ((t == 0) ? 0 : (t == 1) ? 3 : (t == 2) ? 12 : 15) ^ ((a & 1) | ((a & 2) << 1));
-                double af[MB];
+            for (int kq = 0; kq < BK / 16; ++kq) {
 #pragma unroll
-                for (int i = 0; i < MB; ++i) {
-                    const int mg = wm * (C::WM / 16) + (i >> 1);
-                    const int ml = g + 8 * (i & 1);
-                    af[i] = *reinterpret_cast<const double *>(
-                        sa + (mg * BK + k) * 128 + (((ml >> 1) ^ (k & 7)) << 4) + ((ml & 1) << 3));
-                }
+                for (int a = 0; a < 4; ++a) {
+                    double af[MB];
 #pragma unroll
-                for (int j = 0; j < NB; ++j) {
-                    const int n = wn * C::WN + j * 8 + g;
-                    const double b = *reinterpret_cast<const double *>(
-                        sb + n * 128 + ((((k >> 1) & 7) ^ g) << 4) + ((k & 1) << 3));
+                    for (int i = 0; i < MB; ++i) {
+                        const int mg = wm * (C::WM / 16) + (i >> 1);
+                        af[i] = *reinterpret_cast<const double *>(
+                            sa + (mg * BK + kq * 16) * 128 + (real_a_off[a] ^ ((i & 1) << 6)));
+                    }
 #pragma unroll
-                    for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                    for (int j = 0; j < NB; ++j) {
+                        const double b = *reinterpret_cast<const double *>(
+                            sb + (kq * BN + wn * C::WN + j * 8) * 128 + real_b_off[a]);
+#pragma unroll
+                        for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                    }
                 }
             }
         }
@@ -320,7 +337,7 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     {   // A: H viewed as (16 doubles, k, m_group)
         cuuint64_t dims[3] = {16, N, N / C::ROWS128};
         cuuint64_t strides[2] = {N * C::ESZ, 128};
-        cuuint32_t box[3] = {16, BK, (cuuint32_t)(C::BM / C::ROWS128)};
+        cuuint32_t box[3] = {16, (cuuint32_t)C::BK, (cuuint32_t)(C::BM / C::ROWS128)};
         cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = enc((CUtensorMap *)plan->tmap_H, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)plan->H, dims,
                          strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
