@@ -103,6 +103,23 @@ int chase_filter_scalars(double a, double b, double lambda1, int32_t m_max,
                          double *alpha, double *beta, double *c);
 int chase_filter_schedule(const int32_t *degrees, int64_t ncols, int32_t *offset);
 
+/* Degree optimisation, host only (Alg. 5 "Degree Optimization"; Eq. (8),
+ * PAPER.md:358) followed by the sort of Alg. 1 l.15.  For every column j:
+ *     t = (ritzv[j] - c)/e,  c = (a+b)/2, e = (b-a)/2               (Alg. 5 l.2)
+ *     rho = max(|t - sqrt(t^2-1)|, |t + sqrt(t^2-1)|)               (l.3; rho = 1 if |t| <= 1)
+ *     deg = ceil(| ln(resid[j]/tol) / ln(rho) |)                    (l.4)
+ *     deg = min(deg + deg_extra, deg_max)                           (l.5)
+ *     deg = deg + (deg mod 2)                                       (l.6: even)
+ * rho == 1 (Ritz value inside [a,b]) or a non-finite quotient gives deg_max before l.6.
+ * degrees_out[i] (HOST int32[ncols]) receives the degrees sorted ascending, perm_out[i] (HOST
+ * int64[ncols], may be NULL) the original index of the column that must move to position i
+ * (stable sort), i.e. the permutation the caller applies to V, ritzv and resid before
+ * chase_filter.  Returns 0, CHASE_ERR_ARG (null pointer, ncols < 0, tol <= 0, deg_extra < 0,
+ * deg_max < 1, a resid <= 0 or non-finite) or CHASE_ERR_BOUNDS (not a < b, non-finite). */
+int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, double tol,
+                  double a, double b, int32_t deg_extra, int32_t deg_max,
+                  int32_t *degrees_out, int64_t *perm_out);
+
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel,
  * 0 = generic FMA kernel.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);

@@ -96,3 +96,31 @@ def chase_filter(H: np.ndarray, V0: np.ndarray, degrees, a: float, b: float, lam
     if rc != 0:
         raise RuntimeError(f"oracle_chase_filter failed: {rc}")
     return V
+
+
+def chase_degrees(resid, ritzv, tol: float, a: float, b: float, deg_extra: int = 2, deg_max: int = 36):
+    """ORACLE for Alg. 5 "Degree Optimization" (PAPER.md:365-393; Eq. (8), PAPER.md:358) and the
+    sort by degree of Alg. 1 l.15, written line by line in the paper's notation.
+    Returns (deg unsorted [list of int], order [stable argsort by degree]).
+
+    Reading (G17): for |t| <= 1 the two roots t +- sqrt(t^2-1) are complex of modulus 1,
+    so |rho| = 1, log|rho| = 0 and line 4 is unbounded: line 5's cap gives deg = DEGMAX.
+    """
+    import cmath
+    import math
+    c = (a + b) / 2.0
+    e = (b - a) / 2.0
+    deg = []
+    for res, lam in zip(resid, ritzv):
+        t = (lam - c) / e                                                    # l.2
+        root = cmath.sqrt(t * t - 1.0)
+        rho = max(abs(t - root), abs(t + root))                              # l.3
+        if rho <= 1.0 + 1e-300 or math.log(rho) == 0.0:
+            d = float("inf")
+        else:
+            d = math.ceil(abs(math.log(res / tol) / math.log(rho)))          # l.4
+        d = min(d + deg_extra, deg_max)                                      # l.5
+        d = int(d)
+        deg.append(d + d % 2)                                                # l.6
+    order = sorted(range(len(deg)), key=lambda j: deg[j])                    # Alg. 1 l.15 (stable)
+    return deg, order

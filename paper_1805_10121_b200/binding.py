@@ -20,7 +20,7 @@ _DTYPE_CODE = {torch.float32: CHASE_F32, torch.float64: CHASE_F64,
 EXPORTS = [
     "chase_filter", "chase_filter_ws", "chase_filter_host", "chase_filter_workspace_bytes",
     "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
-    "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror",
+    "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
 ]
 
 _lib = None
@@ -66,6 +66,8 @@ def load() -> ctypes.CDLL:
     lib.chase_filter_launch_count.argtypes = []
     lib.chase_fp64_peak_probe.restype = ctypes.c_int
     lib.chase_fp64_peak_probe.argtypes = [ctypes.c_int, ctypes.c_int, vp]
+    lib.chase_degrees.restype = ctypes.c_int
+    lib.chase_degrees.argtypes = [i64, vp, vp, dbl, dbl, dbl, i32, i32, vp, vp]
     lib.chase_filter_strerror.restype = ctypes.c_char_p
     lib.chase_filter_strerror.argtypes = [ctypes.c_int]
     _lib = lib
@@ -206,3 +208,17 @@ def chase_fp64_peak_probe(kind: int, iters: int = 4096) -> float:
     g = ctypes.c_double()
     _check(load().chase_fp64_peak_probe(int(kind), int(iters), ctypes.addressof(g)))
     return g.value
+
+
+def chase_degrees(resid, ritzv, tol: float, a: float, b: float, deg_extra: int = 2, deg_max: int = 36):
+    """Alg. 5 + the sort of Alg. 1 l.15: (degrees sorted ascending [int32], perm [int64]) with
+    degrees[i] belonging to original column perm[i]."""
+    res = np.ascontiguousarray(np.asarray(resid, dtype=np.float64))
+    rv = np.ascontiguousarray(np.asarray(ritzv, dtype=np.float64))
+    if res.shape != rv.shape or res.ndim != 1:
+        raise ValueError("resid and ritzv must be 1-D arrays of equal length")
+    deg = np.zeros(res.size, dtype=np.int32)
+    perm = np.zeros(res.size, dtype=np.int64)
+    _check(load().chase_degrees(res.size, res.ctypes.data, rv.ctypes.data, float(tol), float(a), float(b),
+                                int(deg_extra), int(deg_max), deg.ctypes.data, perm.ctypes.data))
+    return deg, perm

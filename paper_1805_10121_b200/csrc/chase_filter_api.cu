@@ -1,6 +1,7 @@
 // Host orchestration of the Chebyshev filter (Alg. 4) behind the C ABI of
 // include/chase_filter.h: validation, the sigma recurrence (l.2-5, 8, 11), the active-suffix
 // schedule (l.12-14) and one fused step kernel per degree on one CUDA stream.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdlib>
@@ -91,6 +92,41 @@ int chase_filter_schedule(const int32_t *degrees, int64_t ncols, int32_t *offset
         }
     }
     return m_max;
+}
+
+int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, double tol,
+                  double a, double b, int32_t deg_extra, int32_t deg_max,
+                  int32_t *degrees_out, int64_t *perm_out) {
+    if (ncols < 0 || ncols > kMaxDim || !(tol > 0.0) || !std::isfinite(tol) || deg_extra < 0 || deg_max < 1)
+        return CHASE_ERR_ARG;
+    if (ncols > 0 && (!resid || !ritzv || !degrees_out)) return CHASE_ERR_ARG;
+    if (!(std::isfinite(a) && std::isfinite(b)) || !(a < b)) return CHASE_ERR_BOUNDS;
+    const double c = 0.5 * (b + a), e = 0.5 * (b - a);
+    std::vector<int32_t> deg((size_t)ncols);
+    for (int64_t j = 0; j < ncols; ++j) {
+        if (!(resid[j] > 0.0) || !std::isfinite(resid[j]) || !std::isfinite(ritzv[j])) return CHASE_ERR_ARG;
+        const double t = (ritzv[j] - c) / e;                                   // Alg. 5 l.2
+        int32_t d = deg_max;
+        if (std::fabs(t) > 1.0) {
+            const double r = std::sqrt(t * t - 1.0);
+            const double rho = std::fmax(std::fabs(t - r), std::fabs(t + r));   // l.3
+            const double q = std::fabs(std::log(resid[j] / tol) / std::log(rho));   // l.4
+            if (std::isfinite(q) && q < (double)deg_max) {
+                const double dq = std::ceil(q) + (double)deg_extra;             // l.4, l.5
+                d = dq < (double)deg_max ? (int32_t)dq : deg_max;
+            }
+        }
+        deg[(size_t)j] = d + (d & 1);                                           // l.6
+    }
+    std::vector<int64_t> order((size_t)ncols);
+    for (int64_t j = 0; j < ncols; ++j) order[(size_t)j] = j;
+    std::stable_sort(order.begin(), order.end(),
+                     [&](int64_t x, int64_t y) { return deg[(size_t)x] < deg[(size_t)y]; });   // Alg. 1 l.15
+    for (int64_t i = 0; i < ncols; ++i) {
+        degrees_out[i] = deg[(size_t)order[(size_t)i]];
+        if (perm_out) perm_out[i] = order[(size_t)i];
+    }
+    return CHASE_OK;
 }
 
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
