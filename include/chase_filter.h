@@ -120,6 +120,24 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
                   double a, double b, int32_t deg_extra, int32_t deg_max,
                   int32_t *degrees_out, int64_t *perm_out);
 
+/* The other two HEMM call sites of ChASE, on the same step kernels.
+ *
+ * chase_hemm:  Y <- alpha (H - shift I) X + beta Y            (Listing 1 HEMM, PAPER.md:511;
+ *   Rayleigh-Ritz A Q^, Alg. 2 l.2).  H, X, Y DEVICE, column-major, ld = N, 16-byte
+ *   aligned, X and Y distinct N x ncols buffers; beta == 0 means Y is write-only.  Asynchronous.
+ *
+ * chase_residuals:  resid[j] = || H V[:,j] - ritzv[j] V[:,j] ||_2     (Alg. 1 l.8, PAPER.md:160;
+ *   Listing 1 Resd).  One step kernel with a per-column shift in the epilogue
+ *   (R = H V - V diag(ritzv) into the workspace) plus one column-norm kernel.  V DEVICE (read
+ *   only), ritzv HOST double[ncols] (consumed before return), resid DEVICE double[ncols],
+ *   workspace DEVICE >= chase_residuals_workspace_bytes(...).  Asynchronous on `stream`. */
+int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
+               double alpha, double beta, double shift, chase_dtype_t dtype, void *stream);
+size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
+int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, const double *ritzv,
+                    double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
+                    void *stream);
+
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel,
  * 0 = generic FMA kernel.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);

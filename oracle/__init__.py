@@ -124,3 +124,33 @@ def chase_degrees(resid, ritzv, tol: float, a: float, b: float, deg_extra: int =
         deg.append(d + d % 2)                                                # l.6
     order = sorted(range(len(deg)), key=lambda j: deg[j])                    # Alg. 1 l.15 (stable)
     return deg, order
+
+
+def hemm(H: np.ndarray, X: np.ndarray, Y, alpha: float = 1.0, beta: float = 0.0, shift=0.0) -> np.ndarray:
+    """ORACLE: alpha (H X - X diag(shift)) + beta Y in FP64 (Listing 1 HEMM), new array.
+    `shift` is a scalar or one value per column."""
+    lib = _load()
+    lib.oracle_hemm.restype = ctypes.c_int
+    lib.oracle_hemm.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_void_p,
+                                ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_void_p]
+    H = np.asarray(H)
+    if not H.flags.f_contiguous:
+        H = np.asfortranarray(H)
+    is_complex = np.iscomplexobj(H)
+    h_is_f32 = H.dtype in (np.float32, np.complex64)
+    wide = np.complex128 if is_complex else np.float64
+    Xw = np.array(X, dtype=wide, order="F", copy=True)
+    N, n = Xw.shape
+    Yw = np.zeros((N, n), dtype=wide, order="F") if Y is None else np.array(Y, dtype=wide, order="F", copy=True)
+    sh = np.ascontiguousarray(np.broadcast_to(np.asarray(shift, dtype=np.float64), (n,)))
+    rc = lib.oracle_hemm(H.ctypes.data, int(h_is_f32), int(is_complex), N, Xw.ctypes.data, Yw.ctypes.data, n,
+                         float(alpha), float(beta), sh.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"oracle_hemm failed: {rc}")
+    return Yw
+
+
+def residuals(H: np.ndarray, V: np.ndarray, ritzv) -> np.ndarray:
+    """ORACLE: resid[j] = ||H v_j - ritzv[j] v_j||_2 (Alg. 1 l.8; Resd)."""
+    R = hemm(H, V, None, 1.0, 0.0, np.asarray(ritzv, dtype=np.float64))
+    return np.sqrt(np.sum(R.real ** 2 + R.imag ** 2, axis=0))

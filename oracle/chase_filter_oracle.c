@@ -244,3 +244,24 @@ int oracle_chase_filter(const void *H, int h_is_f32, int is_complex, int64_t N,
     free(cur); free(oth); free(src); free(dst);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------
+ * The HEMM of Listing 1 as a general product, with a per-column shift:
+ *     Y[:,j] <- alpha * ( H X[:,j] - shift[j] X[:,j] ) + beta * Y[:,j]
+ * Used for Rayleigh-Ritz's A Q^ (Alg. 2 l.2: alpha=1, beta=0, shift=0) and for
+ * the residual block H V - V diag(ritzv) (Alg. 1 l.8).  Same k-ascending sums
+ * as the filter steps.  X, Y: N x ncols FP64 (interleaved if complex), distinct buffers.
+ * ---------------------------------------------------------------------------------- */
+int oracle_hemm(const void *H, int h_is_f32, int is_complex, int64_t N,
+                const double *X, double *Y, int64_t ncols,
+                double alpha, double beta, const double *shift) {
+    if (!H || !X || !Y || !shift || N <= 0 || ncols < 0) return -1;
+    int64_t ld = (is_complex ? 2 : 1) * N;
+    for (int64_t j = 0; j < ncols; ++j) {       /* one column at a time: its own shift */
+        double *src = (double *)(X + j * ld);
+        double *dst = Y + j * ld;
+        if (is_complex) step_complex(H, h_is_f32, N, 1, &src, &dst, alpha, beta, shift[j]);
+        else            step_real(H, h_is_f32, N, 1, &src, &dst, alpha, beta, shift[j]);
+    }
+    return 0;
+}

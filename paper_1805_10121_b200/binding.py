@@ -21,6 +21,7 @@ EXPORTS = [
     "chase_filter", "chase_filter_ws", "chase_filter_host", "chase_filter_workspace_bytes",
     "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
+    "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes",
 ]
 
 _lib = None
@@ -68,6 +69,12 @@ def load() -> ctypes.CDLL:
     lib.chase_fp64_peak_probe.argtypes = [ctypes.c_int, ctypes.c_int, vp]
     lib.chase_degrees.restype = ctypes.c_int
     lib.chase_degrees.argtypes = [i64, vp, vp, dbl, dbl, dbl, i32, i32, vp, vp]
+    lib.chase_hemm.restype = ctypes.c_int
+    lib.chase_hemm.argtypes = [vp, i64, vp, vp, i64, dbl, dbl, dbl, ctypes.c_int, vp]
+    lib.chase_residuals_workspace_bytes.restype = sz
+    lib.chase_residuals_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
+    lib.chase_residuals.restype = ctypes.c_int
+    lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
     lib.chase_filter_strerror.restype = ctypes.c_char_p
     lib.chase_filter_strerror.argtypes = [ctypes.c_int]
     _lib = lib
@@ -222,3 +229,49 @@ def chase_degrees(resid, ritzv, tol: float, a: float, b: float, deg_extra: int =
     _check(load().chase_degrees(res.size, res.ctypes.data, rv.ctypes.data, float(tol), float(a), float(b),
                                 int(deg_extra), int(deg_max), deg.ctypes.data, perm.ctypes.data))
     return deg, perm
+
+
+def chase_hemm(H: torch.Tensor, X: torch.Tensor, Y: torch.Tensor, alpha: float = 1.0, beta: float = 0.0,
+               shift: float = 0.0, stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """Y <- alpha (H - shift I) X + beta Y on the step kernels (device tensors, column-major)."""
+    if not (H.is_cuda and X.is_cuda and Y.is_cuda):
+        raise ValueError("H, X, Y must be CUDA tensors (there is no CPU path)")
+    if not (H.dtype == X.dtype == Y.dtype) or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H, X, Y must share a dtype in {f32, f64, c64, c128}")
+    for t, nm in ((H, "H"), (X, "X"), (Y, "Y")):
+        _check_colmajor(t, nm)
+    N, ncols = X.shape
+    if H.shape != (N, N) or Y.shape != X.shape:
+        raise ValueError("shape mismatch")
+    with torch.cuda.device(H.device):
+        _check(load().chase_hemm(H.data_ptr(), N, X.data_ptr(), Y.data_ptr(), ncols, float(alpha), float(beta),
+                                 float(shift), _DTYPE_CODE[H.dtype], _stream_ptr(stream)))
+    return Y
+
+
+def chase_residuals_workspace_bytes(N: int, ncols: int, dtype: torch.dtype) -> int:
+    return int(load().chase_residuals_workspace_bytes(N, ncols, _DTYPE_CODE[dtype]))
+
+
+def chase_residuals(H: torch.Tensor, V: torch.Tensor, ritzv, workspace: Optional[torch.Tensor] = None,
+                    stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """resid[j] = ||H V[:,j] - ritzv[j] V[:,j]||_2 as a device float64 tensor [ncols]."""
+    if not (H.is_cuda and V.is_cuda):
+        raise ValueError("H and V must be CUDA tensors (there is no CPU path)")
+    if H.dtype != V.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V, "V")
+    N, ncols = V.shape
+    rv = np.ascontiguousarray(np.asarray(ritzv, dtype=np.float64))
+    if rv.shape != (ncols,):
+        raise ValueError("ritzv must have one entry per column")
+    need = chase_residuals_workspace_bytes(N, ncols, H.dtype)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=H.device)
+    resid = torch.empty(ncols, dtype=torch.float64, device=H.device)
+    with torch.cuda.device(H.device):
+        _check(load().chase_residuals(H.data_ptr(), N, V.data_ptr(), ncols, rv.ctypes.data, resid.data_ptr(),
+                                      _DTYPE_CODE[H.dtype], workspace.data_ptr(),
+                                      workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return resid

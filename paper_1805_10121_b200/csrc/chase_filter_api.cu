@@ -129,6 +129,65 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
     return CHASE_OK;
 }
 
+// One launch of the step kernel family: Y <- alpha (H X - c X) + beta Y with X, Y whole buffers.
+static int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha,
+                           double beta, double c, const double *c_col, int use_beta, chase_dtype_t dtype,
+                           cudaStream_t stream) {
+    if (chase_filter_kernel_path(N, ncols, dtype) == 1) {
+        DmmaPlan plan;
+        cudaError_t e = dmma_plan_create(&plan, dtype, H, N, const_cast<void *>(X), Y, ncols);
+        if (e != cudaSuccess) return (int)e;
+        e = dmma_launch_step(&plan, 0, 0, alpha, beta, c, use_beta, stream, c_col);
+        return (int)e;
+    }
+    StepArgs sa;
+    sa.H = H; sa.X = X; sa.Y = Y; sa.N = N; sa.n = ncols;
+    sa.alpha = alpha; sa.beta = beta; sa.c = c; sa.c_col = c_col; sa.use_beta = use_beta;
+    return (int)launch_step_generic(dtype, sa, stream);
+}
+
+int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
+               double alpha, double beta, double shift, chase_dtype_t dtype, void *stream_) {
+    if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return CHASE_ERR_ARG;
+    if (!H || (ncols > 0 && (!X || !Y || X == Y))) return CHASE_ERR_ARG;
+    if (!(std::isfinite(alpha) && std::isfinite(beta) && std::isfinite(shift))) return CHASE_ERR_ARG;
+    if (ncols == 0) return CHASE_OK;
+    if (((uintptr_t)H | (uintptr_t)X | (uintptr_t)Y) & 15) return CHASE_ERR_ALIGN;
+    return launch_one_step(H, N, X, Y, ncols, alpha, beta, shift, nullptr, beta != 0.0, dtype,
+                           (cudaStream_t)stream_);
+}
+
+size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype) {
+    const size_t v = chase_filter_workspace_bytes(N, ncols, dtype);
+    if (v == 0 && ncols != 0) return 0;
+    return v + ((size_t)ncols * sizeof(double) + 255) / 256 * 256;
+}
+
+int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, const double *ritzv,
+                    double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
+                    void *stream_) {
+    cudaStream_t stream = (cudaStream_t)stream_;
+    if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return CHASE_ERR_ARG;
+    if (!H || (ncols > 0 && (!V || !ritzv || !resid))) return CHASE_ERR_ARG;
+    if (ncols == 0) return CHASE_OK;
+    for (int64_t j = 0; j < ncols; ++j)
+        if (!std::isfinite(ritzv[j])) return CHASE_ERR_ARG;
+    if (!workspace || workspace_bytes < chase_residuals_workspace_bytes(N, ncols, dtype)) return CHASE_ERR_WORKSPACE;
+    if (((uintptr_t)H | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
+    const size_t r_bytes = chase_filter_workspace_bytes(N, ncols, dtype);
+    double *d_shift = (double *)((char *)workspace + r_bytes);
+    // ritzv is consumed before return: stage it through a pinned-free synchronous-safe copy
+    cudaError_t e = cudaMemcpyAsync(d_shift, ritzv, (size_t)ncols * sizeof(double), cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return (int)e;
+    e = cudaStreamSynchronize(stream);      // pageable source: make "consumed before return" true
+    if (e != cudaSuccess) return (int)e;
+    int rc = launch_one_step(H, N, V, workspace, ncols, 1.0, 0.0, 0.0, d_shift, 0, dtype, stream);
+    if (rc != CHASE_OK) return rc;
+    return (int)launch_column_norms(dtype, workspace, N, ncols, resid, stream);
+}
+
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
     if (N <= 0 || ncols < 0) return CHASE_ERR_ARG;

@@ -18,6 +18,7 @@ struct StepArgs {
     int64_t N;
     int64_t n;
     double alpha, beta, c;
+    const double *c_col = nullptr;   // optional per-column shift (device double[n]); overrides c
     int use_beta;
 };
 
@@ -41,7 +42,11 @@ cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H,
                              void *V, void *W, int64_t ncols);
 // Step reading buffer `src` (0/1) and writing buffer 1-src, active columns [s, ncols).
 cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
-                             double c, int use_beta, cudaStream_t stream);
+                             double c, int use_beta, cudaStream_t stream, const double *c_col = nullptr);
+
+// resid[j] = || R[:, j] ||_2 for an N x n column-major block R (device), resid device double[n].
+cudaError_t launch_column_norms(chase_dtype_t dtype, const void *R, int64_t N, int64_t n, double *resid,
+                                cudaStream_t stream);
 
 void count_launch();
 

@@ -106,6 +106,7 @@ struct StepParams {
     int col0;            // first active column in the full buffer (TMA coordinate offset)
     int tiles_m, tiles_n;
     double alpha, beta, c;
+    const double *c_col;   // optional per-column shift (device, indexed by active column); overrides c
     int use_beta;
 };
 
@@ -273,7 +274,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     // ---------------------------------------------------------------- fused epilogue
     // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
-    const double alpha = p.alpha, beta = p.beta, c = p.c;
+    const double alpha = p.alpha, beta = p.beta;
     constexpr int NC = CPLX ? 2 : 1;
 #pragma unroll
     for (int j = 0; j < NB; ++j) {
@@ -281,6 +282,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
         for (int e = 0; e < 2; ++e) {
             const int col = n0 + wn * C::WN + j * 8 + 2 * t + e;
             if (col >= p.n) continue;
+            const double c = p.c_col ? p.c_col[col] : p.c;
 #pragma unroll
             for (int i = 0; i < MB; ++i) {
                 int row;
@@ -359,7 +361,7 @@ cudaError_t encode_maps(DmmaPlan *plan) {
 
 template <bool CPLX>
 cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
-                   cudaStream_t stream) {
+                   cudaStream_t stream, const double *c_col) {
     using C = Cfg<CPLX>;
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
@@ -382,6 +384,7 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     p.alpha = alpha;
     p.beta = beta;
     p.c = c;
+    p.c_col = c_col;
     p.use_beta = use_beta;
     const CUtensorMap *mA = (const CUtensorMap *)plan->tmap_H;
     const CUtensorMap *mB = (const CUtensorMap *)plan->tmap_B[src];
@@ -411,9 +414,9 @@ cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H,
 }
 
 cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c,
-                             int use_beta, cudaStream_t stream) {
-    return plan->dtype == CHASE_C128 ? launch<true>(plan, src, s, alpha, beta, c, use_beta, stream)
-                                     : launch<false>(plan, src, s, alpha, beta, c, use_beta, stream);
+                             int use_beta, cudaStream_t stream, const double *c_col) {
+    return plan->dtype == CHASE_C128 ? launch<true>(plan, src, s, alpha, beta, c, use_beta, stream, c_col)
+                                     : launch<false>(plan, src, s, alpha, beta, c, use_beta, stream, c_col);
 }
 
 }  // namespace chase

@@ -13,7 +13,7 @@ constexpr int kThreads = 256;   // 16 x 16 thread grid; thread (tx, ty) owns row
 template <typename R, bool CPLX, int TM, int TN, int BK>
 __global__ void __launch_bounds__(kThreads)
 step_generic_kernel(const R *__restrict__ H, const R *__restrict__ X, R *Y,
-                    int64_t N, int64_t n, R alpha, R beta, R c, int use_beta) {
+                    int64_t N, int64_t n, R alpha, R beta, R c0, const double *__restrict__ c_col, int use_beta) {
     constexpr int BM = 16 * TM, BN = 16 * TN;
     constexpr int NC = CPLX ? 2 : 1;
     __shared__ R As[NC][BK][BM];
@@ -93,6 +93,7 @@ step_generic_kernel(const R *__restrict__ H, const R *__restrict__ X, R *Y,
     for (int j = 0; j < TN; ++j) {
         const int64_t gj = n0 + ty + 16 * j;
         if (gj >= n) continue;
+        const R c = c_col ? (R)c_col[gj] : c0;
 #pragma unroll
         for (int i = 0; i < TM; ++i) {
             const int64_t gm = m0 + tx + 16 * i;
@@ -114,12 +115,47 @@ cudaError_t launch(const StepArgs &a, cudaStream_t stream) {
     dim3 grid((unsigned)((a.N + BM - 1) / BM), (unsigned)((a.n + BN - 1) / BN));
     if (grid.y > 65535) return cudaErrorInvalidConfiguration;
     step_generic_kernel<R, CPLX, TM, TN, BK><<<grid, kThreads, 0, stream>>>(
-        (const R *)a.H, (const R *)a.X, (R *)a.Y, a.N, a.n, (R)a.alpha, (R)a.beta, (R)a.c, a.use_beta);
+        (const R *)a.H, (const R *)a.X, (R *)a.Y, a.N, a.n, (R)a.alpha, (R)a.beta, (R)a.c, a.c_col, a.use_beta);
     count_launch();
     return cudaGetLastError();
 }
 
 }  // namespace
+
+namespace {
+// one CTA per column: sum of |r|^2 in FP64, then sqrt
+template <typename R, int NC>
+__global__ void __launch_bounds__(256) column_norms_kernel(const R *__restrict__ Rm, int64_t N, double *resid) {
+    const R *col = Rm + (int64_t)blockIdx.x * N * NC;
+    double s = 0.0;
+    for (int64_t i = threadIdx.x; i < N * NC; i += blockDim.x) {
+        const double v = (double)col[i];
+        s = fma(v, v, s);
+    }
+    __shared__ double red[256];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (threadIdx.x < w) red[threadIdx.x] += red[threadIdx.x + w];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) resid[blockIdx.x] = sqrt(red[0]);
+}
+}  // namespace
+
+cudaError_t launch_column_norms(chase_dtype_t dtype, const void *Rm, int64_t N, int64_t n, double *resid,
+                                cudaStream_t stream) {
+    if (n <= 0) return cudaSuccess;
+    switch (dtype) {
+        case CHASE_F32: column_norms_kernel<float, 1><<<(unsigned)n, 256, 0, stream>>>((const float *)Rm, N, resid); break;
+        case CHASE_F64: column_norms_kernel<double, 1><<<(unsigned)n, 256, 0, stream>>>((const double *)Rm, N, resid); break;
+        case CHASE_C64: column_norms_kernel<float, 2><<<(unsigned)n, 256, 0, stream>>>((const float *)Rm, N, resid); break;
+        case CHASE_C128: column_norms_kernel<double, 2><<<(unsigned)n, 256, 0, stream>>>((const double *)Rm, N, resid); break;
+        default: return cudaErrorInvalidValue;
+    }
+    count_launch();
+    return cudaGetLastError();
+}
 
 cudaError_t launch_step_generic(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream) {
     if (a.n <= 0) return cudaSuccess;
