@@ -62,8 +62,10 @@ enum {
     CHASE_ERR_ALIGN = -6      /* H, V or workspace not aligned to 16 bytes */
 };
 
-/* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype`
- * (the W of Alg. 4), rounded up to 256 bytes.  0 if an argument is invalid. */
+/* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype` (the W of
+ * Alg. 4), rounded up to 256 bytes; on the tcgen05 3xTF32 path (see chase_filter_kernel_path)
+ * three such buffers plus one N x N buffer (low-order parts of the iterates and of H).
+ * 0 if an argument is invalid. */
 size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
 /* The filter with caller-provided scratch.
@@ -138,8 +140,11 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
                     double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
                     void *stream);
 
-/* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel,
- * 0 = generic FMA kernel.  Negative = invalid arguments. */
+/* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
+ * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 16 == 0, f32 with
+ * N % 32 == 0; needs the larger workspace chase_filter_workspace_bytes reports), 0 = generic FMA
+ * kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1 turns 2
+ * into 0.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
 /* Number of kernels launched by this library since load (all streams); for bench.py. */

@@ -49,8 +49,12 @@ int64_t chase_filter_launch_count(void) { return g_launches.load(); }
 size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     size_t w = elem_bytes(dtype);
     if (w == 0 || N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return 0;
-    size_t bytes = (size_t)N * (size_t)ncols * w;
-    return (bytes + 255) / 256 * 256;
+    size_t bytes = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
+    if (chase_filter_kernel_path(N, ncols, dtype) == 2) {
+        // tcgen05 3xTF32 path: W, lo parts (complex: also -i V and its lo part) and H_lo (N x N)
+        bytes = (size_t)tf32_vector_blocks(dtype) * bytes + ((size_t)N * (size_t)N * w + 255) / 256 * 256;
+    }
+    return bytes;
 }
 
 int chase_filter_scalars(double a, double b, double lambda1, int32_t m_max,
@@ -193,7 +197,10 @@ int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     if (N <= 0 || ncols < 0) return CHASE_ERR_ARG;
     const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
     if (force && force[0] == '1') return 0;
-    return dmma_supported(N, ncols, dtype) ? 1 : 0;
+    if (dmma_supported(N, ncols, dtype)) return 1;
+    const char *no_tf32 = std::getenv("CHASE_FILTER_NO_TF32");
+    if (tf32_supported(N, ncols, dtype) && !(no_tf32 && no_tf32[0] == '1')) return 2;
+    return 0;
 }
 
 int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
@@ -226,10 +233,17 @@ int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int3
     void *buf[2] = {V, workspace};
     const size_t col_bytes = (size_t)N * w;
 
-    const bool use_dmma = chase_filter_kernel_path(N, ncols, dtype) == 1;
+    const int path = chase_filter_kernel_path(N, ncols, dtype);
+    const bool use_dmma = path == 1, use_tf32 = path == 2;
     DmmaPlan plan;
+    Tf32Plan tplan;
     if (use_dmma) {
         cudaError_t e = dmma_plan_create(&plan, dtype, H, N, V, workspace, ncols);
+        if (e != cudaSuccess) return (int)e;
+    }
+    if (use_tf32) {
+        const size_t vb = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
+        cudaError_t e = tf32_plan_create(&tplan, dtype, H, N, V, workspace, vb, ncols, stream);
         if (e != cudaSuccess) return (int)e;
     }
 
@@ -239,6 +253,8 @@ int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int3
         cudaError_t e;
         if (use_dmma) {
             e = dmma_launch_step(&plan, src, s, alpha[k], beta[k], c, k > 1, stream);
+        } else if (use_tf32) {
+            e = tf32_launch_step(&tplan, src, s, alpha[k], beta[k], c, k > 1, stream);
         } else {
             StepArgs sa;
             sa.H = H;

@@ -1,0 +1,454 @@
+// tcgen05 (5th-gen tensor core) step kernel for float32 / complex64: 3xTF32 split products with
+// FP32 accumulation in TMEM.
+//
+//   Y[:, j] <- alpha * (H X[:, j] - c X[:, j]) + beta * Y[:, j]     (Alg. 4 l.4 / l.9; Eq. 7)
+//
+// Every fp32 operand x is split as x = hi + lo, hi = x with the low 13 mantissa bits cleared
+// (what kind::tf32 reads from an fp32 word), lo = x - hi (exact in fp32).  The product is
+// evaluated as hi*lo + lo*hi + hi*hi (lo*lo ~ 2^-22 relative is dropped): three tcgen05.mma per
+// k-slice into ONE fp32 accumulator in tensor memory, which restores fp32-level accuracy (plain
+// single-pass TF32, 2^-11 per operand, would not meet the 1e-4 bound).  The lo parts live in
+// global memory: H_lo is computed once per chase_filter call, the lo part of each new iterate is
+// written by the epilogue that produces it.
+//
+// Both operands are K-major.  For A this uses that H is Hermitian (reading G9): row m of
+// H along k is the conjugate of column m, which is contiguous in the column-major storage.
+//   float32:   A[m][k] = H[k][m] (column m read along k); B = X as stored; D = 128 rows x 256 columns.
+//   complex64: a REAL GEMM over the interleaved index kk = 2k + {0, 1}:
+//     A2[m][kk]  = column m of H as floats    = (Re A[m,k], -Im A[m,k])      (conjugate of H[k,m])
+//     B1[kk][j]  = column j of X as floats    = (Re x, Im x)
+//     B2[kk][j]  = column j of Xrot = -i X    = (Im x, -Re x)
+//     A2 . B1 = Re(A x),  A2 . B2 = Im(A x):  D = 128 complex rows x [128 Re | 128 Im] columns.
+//   Xrot (and the lo parts) of every iterate are written by the epilogue that produces it.
+//
+// Warp roles (320 threads, 1 CTA / SM): warp 0 = TMA producer (one lane), warp 1 = TMEM
+// allocator + MMA issuer (one lane), warps 2-9 = accumulator/epilogue warps (TMEM lane quarter =
+// warp % 4, column half = (warp-2)/4).  The MMA issuer accumulates CHUNK stages into one of two
+// TMEM buffers; the accumulator warps add each finished chunk into fp32 registers (round to
+// nearest) while the tensor core fills the other buffer, then run the fused epilogue.
+// Shared-memory operand tiles are the canonical K-major SWIZZLE_64B UMMA layout written directly
+// by TMA: [row][16 floats of k] (64-byte rows, 8-row groups 512 B apart); one UMMA consumes 8 k.
+#include <cuda.h>
+
+#include <mutex>
+
+#include "chase_internal.h"
+
+namespace chase {
+namespace {
+
+constexpr int kAccWarps = 8;       // accumulator / epilogue warps: 4 TMEM lane quarters x 2 column halves
+constexpr int kThreads = (2 + kAccWarps) * 32;
+constexpr int KS = 16;            // floats of k per pipeline stage (two UMMA K = 8 slices)
+constexpr int TM = 128;           // (complex or real) rows per CTA tile = TMEM lanes
+constexpr int TN = 256;           // real B columns per CTA tile = TMEM columns
+constexpr int STAGES = 4;
+constexpr int CHUNK = 2;            // pipeline stages accumulated in TMEM before the sum moves to registers
+constexpr int A_BYTES = TM * KS * 4;          // 8 KB
+constexpr int B_BYTES = TN * KS * 4;          // 16 KB
+constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi + lo of both: 48 KB
+constexpr int SMEM_TOTAL = STAGES * STAGE_BYTES + 1024 + 256;
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+
+// UMMA shared-memory matrix descriptor (sm_100): start address, leading / stride byte offsets
+// (all >> 4), version = 1, layout type in bits 61..63 (2 = SWIZZLE_128B, 4 = SWIZZLE_64B).
+__device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
+    return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
+}
+// Instruction descriptor, kind::tf32: D fp32 (bits 4-5 = 1), A/B TF32 (bits 7-9, 10-12 = 2),
+// A and B K-major (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28.
+constexpr uint32_t kInstrDesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) |
+                                ((uint32_t)(TM >> 4) << 24);
+
+__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+    uint32_t r[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+
+
+struct Tf32Params {
+    const float *X;                     // source iterate, first active column
+    float *Y, *Y_lo, *Yrot, *Yrot_lo;   // destination iterate, its lo part, -i*iterate and its lo part (rot: complex only)
+    int64_t N;                          // matrix order
+    int64_t KF;                         // floats along k per column: 2N (complex) or N (real)
+    int n;                              // active columns
+    int col0;                           // first active column in the full buffers (TMA coordinate offset)
+    int tiles_m, tiles_n;
+    float alpha, beta, c;
+    const double *c_col;
+    int use_beta;
+};
+
+constexpr int kGroupN = 8;
+__device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
+    const int per_group = kGroupN * tiles_m;
+    const int grp = t / per_group;
+    const int first_n = grp * kGroupN;
+    const int gn = min(kGroupN, tiles_n - first_n);
+    const int r = t - grp * per_group;
+    tm = r / gn;
+    tn = first_n + r % gn;
+}
+
+template <bool CPLX>
+__global__ void __launch_bounds__(kThreads, 1)
+step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_constant__ CUtensorMap tmapA_lo,
+                 const __grid_constant__ CUtensorMap tmapB_hi, const __grid_constant__ CUtensorMap tmapB_lo,
+                 const __grid_constant__ CUtensorMap tmapR_hi, const __grid_constant__ CUtensorMap tmapR_lo,
+                 const Tf32Params p) {
+    constexpr int COLS = CPLX ? TN / 2 : TN;      // (complex or real) columns per tile
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[S], empty[S], tfull[2], tempty[2], tmem slot
+    const uint32_t bar_tfull = bar_base + 8 * (2 * STAGES);
+    const uint32_t bar_tempty = bar_base + 8 * (2 * STAGES + 2);
+    const uint32_t tmem_slot = bar_base + 8 * (2 * STAGES + 4);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    int tile_m, tile_n;
+    tile_coords(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
+    const int m0 = tile_m * TM, n0 = tile_n * COLS;
+    const int KT = (int)((p.KF + KS - 1) / KS);          // pipeline stages over k
+    const int NCH = (KT + CHUNK - 1) / CHUNK;            // TMEM accumulation chunks
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(bar_base + 8 * s, 1);              // full: producer's expect_tx arrive
+            mbar_init(bar_base + 8 * (STAGES + s), 1);   // empty: one tcgen05.commit arrive
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_tfull + 8 * b, 1);             // chunk accumulator complete (tcgen05.commit)
+            mbar_init(bar_tempty + 8 * b, kAccWarps);    // chunk accumulator drained by every accumulator warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {   // all of TMEM: two 256-column fp32 accumulators (ping-pong between chunks)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(2 * TN) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ TMA producer
+        if (lane == 0) {
+            for (int kt = 0; kt < KT; ++kt) {
+                const int s = kt % STAGES;
+                const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
+                if (kt >= STAGES) mbar_wait(empty, ((kt / STAGES) - 1) & 1);
+                const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
+                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
+                mbar_expect_tx(full, STAGE_BYTES);
+                const int k0 = kt * KS;
+                tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);          // 128 columns of H, 16 floats of k
+                tma_load_2d(sa_lo, &tmapA_lo, full, k0, m0);
+                tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
+                tma_load_2d(sb_lo, &tmapB_lo, full, k0, p.col0 + n0);
+                if (CPLX) {   // rows 128..255 of the B tile: -i X  (gives the imaginary part of A x)
+                    tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
+                    tma_load_2d(sb_lo + B_BYTES / 2, &tmapR_lo, full, k0, p.col0 + n0);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            int kt = 0;
+            for (int ch = 0; ch < NCH; ++ch) {
+                const int b = ch & 1;
+                if (ch >= 2) {   // the accumulator warps must have drained this buffer's previous chunk
+                    mbar_wait(bar_tempty + 8 * b, ((ch >> 1) - 1) & 1);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                }
+                const uint32_t d = tmem_base + b * TN;
+                const int kt_end = min(KT, kt + CHUNK);
+                for (bool first = true; kt < kt_end; ++kt) {
+                    const int s = kt % STAGES;
+                    mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
+                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
+                    const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
+#pragma unroll
+                    for (int ks = 0; ks < KS / 8; ++ks) {
+                        // K-major SWIZZLE_64B: 8-row groups 512 B apart; the 8-k slice ks starts 32 B into the row
+                        const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
+                        const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
+                        const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
+                        const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
+                        umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
+                        umma_tf32(d, al, bh, 1u);                 // lo * hi
+                        umma_tf32(d, ah, bh, 1u);                 // hi * hi
+                        first = false;
+                    }
+                    umma_commit(bar_base + 8 * (STAGES + s));   // frees the smem stage when these MMAs retire
+                }
+                umma_commit(bar_tfull + 8 * b);                  // this chunk's accumulator is complete
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------ accumulator / epilogue warps
+        // The tensor core's fp32 accumulation rounds toward zero, a bias that grows with the length
+        // of the accumulation chain; so the chain is cut into chunks of CHUNK stages, and the chunk
+        // sums are added here in registers with round-to-nearest.
+        const int quarter = warp & 3;                       // TMEM lanes this warp may access
+        const int half = (warp - 2) >> 2;                   // which 128 of the 256 accumulator columns
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
+        float racc[TN / 2];
+#pragma unroll
+        for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
+        for (int ch = 0; ch < NCH; ++ch) {
+            const int b = ch & 1;
+            mbar_wait(bar_tfull + 8 * b, (ch >> 1) & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int j = 0; j < TN / 2 / 32; ++j) {
+                float t[32];
+                tmem_ld32(taddr + b * TN + j * 32, t);
+#pragma unroll
+                for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_tempty + 8 * b);
+        }
+
+        const int64_t row = (int64_t)m0 + quarter * 32 + lane;
+        const bool row_ok = row < p.N;
+        const float alpha = p.alpha, beta = p.beta;
+#pragma unroll
+        for (int i = 0; i < TN / 2; ++i) {
+            // complex: half 0 owns the real parts, half 1 the imaginary parts of columns n0 .. n0+127
+            const int col = CPLX ? n0 + i : n0 + half * (TN / 2) + i;
+            if (col < p.n && row_ok) {
+                const float c = p.c_col ? (float)p.c_col[col] : p.c;
+                const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
+                float y = alpha * (racc[i] - c * p.X[off]);
+                if (p.use_beta) y = fmaf(beta, p.Y[off], y);
+                const float lo = y - tf32_hi(y);
+                p.Y[off] = y;
+                p.Y_lo[off] = lo;
+                if (CPLX) {   // -i y = (Im y, -Re y)
+                    const int64_t roff = off + (half ? -1 : 1);
+                    p.Yrot[roff] = half ? y : -y;
+                    p.Yrot_lo[roff] = half ? lo : -lo;
+                }
+            }
+        }
+    }
+
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(2 * TN) : "memory");
+    }
+}
+
+// Pre-passes, once per call.  lo[i] = x[i] - hi(x[i]) (H, and a real V0) ...
+__global__ void __launch_bounds__(256) split_lo_kernel(const float *__restrict__ x, float *__restrict__ lo, int64_t count) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) {
+        const float v = x[i];
+        lo[i] = v - tf32_hi(v);
+    }
+}
+// ... and for a complex V0 also rot = -i x and its lo part.
+__global__ void __launch_bounds__(256) split_rot_kernel(const float2 *__restrict__ x, float2 *__restrict__ lo,
+                                                         float2 *__restrict__ rot, float2 *__restrict__ rot_lo,
+                                                         int64_t count) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) {
+        const float2 v = x[i];
+        const float lr = v.x - tf32_hi(v.x), li = v.y - tf32_hi(v.y);
+        lo[i] = make_float2(lr, li);
+        rot[i] = make_float2(v.y, -v.x);
+        rot_lo[i] = make_float2(li, -lr);
+    }
+}
+
+// ---------------------------------------------------------------- host side
+using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                   CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+    });
+    return fn;
+}
+
+// A column-major float matrix (KF floats per column, `cols` columns) viewed K-major:
+// box = 16 floats of k x `box_rows` columns, SWIZZLE_64B.
+cudaError_t encode_kmajor(CUtensorMap *map, const void *base, int64_t KF, int64_t cols, int box_rows) {
+    EncodeTiledFn enc = get_encode_fn();
+    if (!enc) return cudaErrorNotSupported;
+    cuuint64_t dims[2] = {(cuuint64_t)KF, (cuuint64_t)cols};
+    cuuint64_t strides[1] = {(cuuint64_t)KF * 4};
+    cuuint32_t box[2] = {16, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void *>(base), dims, strides, box, estr,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <bool CPLX>
+cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
+                   cudaStream_t stream, const double *c_col) {
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(step_tf32_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL);
+    });
+    if (attr_err != cudaSuccess) return attr_err;
+    const int64_t n = plan->ncols - s;
+    if (n <= 0) return cudaSuccess;
+    constexpr int COLS = CPLX ? TN / 2 : TN;
+    constexpr int FL = CPLX ? 2 : 1;
+    const size_t col_floats = (size_t)plan->N * FL;
+    const int dst = src ^ 1;
+    Tf32Params p;
+    p.X = (const float *)plan->buf[src] + (size_t)s * col_floats;
+    p.Y = (float *)plan->buf[dst] + (size_t)s * col_floats;
+    p.Y_lo = (float *)plan->lo[dst] + (size_t)s * col_floats;
+    p.Yrot = CPLX ? (float *)plan->rot[dst] + (size_t)s * col_floats : nullptr;
+    p.Yrot_lo = CPLX ? (float *)plan->rot_lo[dst] + (size_t)s * col_floats : nullptr;
+    p.N = plan->N;
+    p.KF = plan->N * FL;
+    p.n = (int)n;
+    p.col0 = (int)s;
+    p.tiles_m = (int)((plan->N + TM - 1) / TM);
+    p.tiles_n = (int)((n + COLS - 1) / COLS);
+    p.alpha = (float)alpha;
+    p.beta = (float)beta;
+    p.c = (float)c;
+    p.c_col = c_col;
+    p.use_beta = use_beta;
+    const CUtensorMap *B = (const CUtensorMap *)plan->tmap_B[0];   // [hi V, hi W, lo V, lo W, rot V, rot W, rot_lo V, rot_lo W]
+    const int r_hi = CPLX ? 4 + src : src, r_lo = CPLX ? 6 + src : 2 + src;
+    step_tf32_kernel<CPLX><<<(unsigned)(p.tiles_m * p.tiles_n), kThreads, SMEM_TOTAL, stream>>>(
+        *(const CUtensorMap *)plan->tmap_A[0], *(const CUtensorMap *)plan->tmap_A[1], B[src], B[2 + src], B[r_hi],
+        B[r_lo], p);
+    count_launch();
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
+    if (ncols < 1 || N < 16 || N > (1 << 28) || ncols > (1 << 28)) return false;
+    if (dtype == CHASE_C64) return N % 2 == 0;     // TMA: column stride must be a multiple of 16 bytes
+    if (dtype == CHASE_F32) return N % 4 == 0;
+    return false;
+}
+
+// Workspace layout: [W | V_lo | W_lo | (complex: Vrot | Wrot | Vrot_lo | Wrot_lo) | H_lo], vector blocks of vb bytes.
+int tf32_vector_blocks(chase_dtype_t dtype) { return dtype == CHASE_C64 ? 7 : 3; }
+
+cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V,
+                             void *workspace, size_t vb, int64_t ncols, cudaStream_t stream) {
+    const bool cplx = dtype == CHASE_C64;
+    const int FL = cplx ? 2 : 1;
+    const int64_t KF = N * FL;
+    char *base = (char *)workspace;
+    plan->dtype = dtype;
+    plan->N = N;
+    plan->ncols = ncols;
+    plan->buf[0] = V;            plan->buf[1] = base;
+    plan->lo[0] = base + vb;     plan->lo[1] = base + 2 * vb;
+    if (cplx) {
+        plan->rot[0] = base + 3 * vb;     plan->rot[1] = base + 4 * vb;
+        plan->rot_lo[0] = base + 5 * vb;  plan->rot_lo[1] = base + 6 * vb;
+    } else {
+        plan->rot[0] = plan->rot[1] = plan->rot_lo[0] = plan->rot_lo[1] = nullptr;
+    }
+    void *H_lo = base + (size_t)tf32_vector_blocks(dtype) * vb;
+
+    // lo part of H (x - tf32(x)) and, for V_0, lo (and -i V_0 with its lo part)
+    split_lo_kernel<<<148 * 8, 256, 0, stream>>>((const float *)H, (float *)H_lo, N * KF);
+    count_launch();
+    if (cplx)
+        split_rot_kernel<<<148 * 8, 256, 0, stream>>>((const float2 *)V, (float2 *)plan->lo[0], (float2 *)plan->rot[0],
+                                                       (float2 *)plan->rot_lo[0], N * ncols);
+    else
+        split_lo_kernel<<<148 * 8, 256, 0, stream>>>((const float *)V, (float *)plan->lo[0], N * ncols);
+    count_launch();
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+
+    if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A[0], H, KF, N, TM)) != cudaSuccess) return e;
+    if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A[1], H_lo, KF, N, TM)) != cudaSuccess) return e;
+    void *bufs[8] = {plan->buf[0], plan->buf[1], plan->lo[0], plan->lo[1],
+                     plan->rot[0], plan->rot[1], plan->rot_lo[0], plan->rot_lo[1]};
+    for (int i = 0; i < (cplx ? 8 : 4); ++i)
+        if ((e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], bufs[i], KF, ncols, cplx ? TN / 2 : TN)) != cudaSuccess)
+            return e;
+    return cudaSuccess;
+}
+
+cudaError_t tf32_launch_step(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c,
+                             int use_beta, cudaStream_t stream, const double *c_col) {
+    return plan->dtype == CHASE_C64 ? launch<true>(plan, src, s, alpha, beta, c, use_beta, stream, c_col)
+                                    : launch<false>(plan, src, s, alpha, beta, c, use_beta, stream, c_col);
+}
+
+}  // namespace chase
