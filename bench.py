@@ -41,6 +41,18 @@ UNIT = "GFLOP/s"
 # The DMMA.8x8x4 and DFMA pipes have the same rate; a register-only probe run live below
 # (chase_fp64_peak_probe) measures it on this very GPU.
 FP64_FLOP_PER_CLK_SM = 128
+TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks: tf32 1.1, bf16 2.25 PFLOP/s
+
+
+def measured_bf16_sustained_tflops():
+    """(TFLOP/s, source): the driver-written sustained bf16 GEMM rate (the step kernel is timed inside a
+    long step), else the nominal dense figure."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            m = json.load(f)
+        return float(m["bf16_tflops_sustained"]), "MEASURED_PEAKS.json bf16_tflops_sustained"
+    except (OSError, KeyError, ValueError):
+        return 2250.0, "nominal bf16 dense 2250 TFLOP/s (MEASURED_PEAKS.json absent)"
 
 
 def parse_args():
@@ -303,21 +315,30 @@ def run_ours(args):
     # ---- roofline of the step kernel (all launches of a step are the same kernel) --------------
     sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
     sms = torch.cuda.get_device_properties(device).multi_processor_count
-    peak_nominal = sms * FP64_FLOP_PER_CLK_SM * sm_max_mhz * 1e6 * 1e-12        # TFLOP/s
     probe_dmma = pkg.chase_fp64_peak_probe(1, 1 << 16) * 1e-3
     probe_dfma = pkg.chase_fp64_peak_probe(0, 1 << 16) * 1e-3
     achieved = flops_step * args.steps / (sum(e0.elapsed_time(e1) for e0, e1 in events) * 1e-3) * 1e-12
     kernel_path = pkg.chase_filter_kernel_path(N, n, dtype)
     is_f64 = dtype in (torch.complex128, torch.float64)
-    if not is_f64:
-        peak_nominal *= 2.0       # FP32 FMA pipe: 256 flop/clk/SM
+    if kernel_path == 2:
+        # tcgen05 kind::tf32, three MMAs per algorithmic product (3xTF32): the peak for ALGORITHMIC
+        # flops is a third of the TF32 tensor peak; TF32 peak = measured bf16 GEMM x nominal ratio.
+        bf16, src = measured_bf16_sustained_tflops()
+        peak = bf16 * TF32_OVER_BF16_NOMINAL / 3.0
+        bound, kname = "tensor", "step_tf32_kernel"
+        peak_source = (f"{src} x nominal tf32/bf16 ratio {TF32_OVER_BF16_NOMINAL:.3f} / 3 MMAs per product "
+                       f"(3xTF32 split, DESIGN.md 6.4)")
+    else:
+        per_clk = FP64_FLOP_PER_CLK_SM * (1 if is_f64 else 2)     # FP32 FMA pipe: 256 flop/clk/SM
+        peak = sms * per_clk * sm_max_mhz * 1e6 * 1e-12            # TFLOP/s
+        bound = "tensor" if kernel_path == 1 else "alu"
+        kname = "step_dmma_kernel" if kernel_path == 1 else "step_generic_kernel"
+        peak_source = (f"{sms} SMs x {per_clk} flop/clk/SM x clocks.max.sm {sm_max_mhz:.0f} MHz "
+                       f"(DESIGN.md 'Peak'); MEASURED_PEAKS.json has no FP64 entry")
     roofline = {
-        "bound": "tensor" if kernel_path == 1 else "alu",
-        "kernel": "step_dmma_kernel" if kernel_path == 1 else "step_generic_kernel",
-        "achieved": achieved, "peak": peak_nominal, "unit": "TFLOP/s", "frac": achieved / peak_nominal,
-        "traffic": None,
-        "peak_source": f"{sms} SMs x {FP64_FLOP_PER_CLK_SM * (1 if is_f64 else 2)} flop/clk/SM x clocks.max.sm "
-                       f"{sm_max_mhz:.0f} MHz (DESIGN.md 'Peak'); MEASURED_PEAKS.json has no FP64 entry",
+        "bound": bound, "kernel": kname,
+        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "traffic": None, "peak_source": peak_source,
         "peak_probe_dmma_tflops": probe_dmma, "peak_probe_dfma_tflops": probe_dfma,
         "frac_of_probe_dmma": achieved / probe_dmma if is_f64 else None,
         "frac_of_nvidia_quoted_40tf": achieved / 40.0 if is_f64 else None,

@@ -141,11 +141,18 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
                     void *stream);
 
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
- * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 16 == 0, f32 with
- * N % 32 == 0; needs the larger workspace chase_filter_workspace_bytes reports), 0 = generic FMA
+ * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
+ * N % 4 == 0; needs the larger workspace chase_filter_workspace_bytes reports), 0 = generic FMA
  * kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1 turns 2
  * into 0.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
+
+/* Column tiling the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active` columns
+ * on a GPU with `sms` SMs (host only, no CUDA call; for tests and inspection).  out (HOST int32[4]) =
+ * {row tiles of 128, column tiles of the full width (64 complex128 / 128 float64 columns), narrow
+ * column tiles launched after them, width of a narrow tile}.  The tiles cover columns
+ * [0, n_active) exactly once.  Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
+int chase_filter_step_tiling(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out);
 
 /* Number of kernels launched by this library since load (all streams); for bench.py. */
 int64_t chase_filter_launch_count(void);

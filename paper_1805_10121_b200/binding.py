@@ -21,7 +21,7 @@ EXPORTS = [
     "chase_filter", "chase_filter_ws", "chase_filter_host", "chase_filter_workspace_bytes",
     "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
-    "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes",
+    "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_tiling",
 ]
 
 _lib = None
@@ -75,6 +75,8 @@ def load() -> ctypes.CDLL:
     lib.chase_residuals_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
     lib.chase_residuals.restype = ctypes.c_int
     lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
+    lib.chase_filter_step_tiling.restype = ctypes.c_int
+    lib.chase_filter_step_tiling.argtypes = [i64, i64, ctypes.c_int, i32, vp]
     lib.chase_filter_strerror.restype = ctypes.c_char_p
     lib.chase_filter_strerror.argtypes = [ctypes.c_int]
     _lib = lib
@@ -208,6 +210,13 @@ def chase_filter_schedule(degrees: Sequence[int]):
     offset = np.zeros(m_max + 1, dtype=np.int32)
     lib.chase_filter_schedule(deg.ctypes.data, deg.size, offset.ctypes.data)
     return m_max, offset
+
+
+def chase_filter_step_tiling(N: int, n_active: int, dtype: torch.dtype, sms: int = 148):
+    """(row tiles, full-width column tiles, narrow column tiles, narrow tile width) of one launch."""
+    out = np.zeros(4, dtype=np.int32)
+    _check(load().chase_filter_step_tiling(int(N), int(n_active), _DTYPE_CODE[dtype], int(sms), out.ctypes.data))
+    return tuple(int(x) for x in out)
 
 
 def chase_fp64_peak_probe(kind: int, iters: int = 4096) -> float:

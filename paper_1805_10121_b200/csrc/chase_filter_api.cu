@@ -203,6 +203,14 @@ int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     return 0;
 }
 
+int chase_filter_step_tiling(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out) {
+    if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || n_active <= 0 || N > kMaxDim || n_active > kMaxDim || sms <= 0 || !out) return CHASE_ERR_ARG;
+    if (dtype != CHASE_C128 && dtype != CHASE_F64) return CHASE_ERR_DTYPE;
+    dmma_plan_tiling(N, n_active, dtype, sms, out);
+    return CHASE_OK;
+}
+
 int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                     double a, double b, double lambda1, chase_dtype_t dtype,
                     void *workspace, size_t workspace_bytes, void *stream_) {

@@ -36,6 +36,9 @@ struct DmmaPlan {
     void *buf[2];
 };
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
+// Column tiling one launch on `n` active columns would use on `sms` SMs:
+// out = {row tiles, full-width column tiles, narrow column tiles, narrow tile width}.
+void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_t out[4]);
 // Returns cudaSuccess, or an error (then the caller falls back to the generic kernels
 // only if the failure is "driver entry point unavailable"; anything else is reported).
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N,

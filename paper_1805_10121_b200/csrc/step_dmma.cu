@@ -20,7 +20,10 @@
 // k = {0,3,12,15}[t] ^ {0,1,4,5}[a]), identically for A and B.
 #include <cuda.h>
 
+#include <algorithm>
+#include <cmath>
 #include <mutex>
+#include <vector>
 
 #include "chase_internal.h"
 
@@ -104,7 +107,10 @@ struct StepParams {
     int64_t N;           // matrix order
     int n;               // active columns
     int col0;            // first active column in the full buffer (TMA coordinate offset)
-    int tiles_m, tiles_n;
+    int tiles_m;
+    int tiles_wide;      // column tiles of the full width BN, covering columns [0, tiles_wide * BN)
+    int tiles_narrow;    // column tiles of width narrow_w covering the remaining columns
+    int narrow_w;        // multiple of 8 * WARPS_N, <= BN
     double alpha, beta, c;
     const double *c_col;   // optional per-column shift (device, indexed by active column); overrides c
     int use_beta;
@@ -125,6 +131,101 @@ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int
     tn = first_n + r % gn;
 }
 
+// The k loop of one consumer warp.  FULL = every 8-column block of the warp is valid (the common
+// case: no per-block test, so the compiler schedules loads and MMAs across blocks); otherwise only
+// the first jmax blocks are computed (ragged / narrow tiles).
+template <bool CPLX, bool FULL>
+__device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::WM / 8][Cfg<CPLX>::WN / 8][2],
+                                         const unsigned char *smem, uint32_t bar_base, int KT, int lane, int warp,
+                                         int jmax) {
+    using C = Cfg<CPLX>;
+    using S = Smem<CPLX>;
+    constexpr int BN = C::BN, BK = C::BK, STAGES = C::STAGES;
+    constexpr int MB = C::WM / 8, NB = C::WN / 8;
+    constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
+    const int g = lane >> 2, t = lane & 3;
+    const int wm = warp % C::WARPS_M, wn = warp / C::WARPS_M;
+
+    // float64: lane-dependent byte offsets of the fragment loads, hoisted out of the k loop.
+    // MMA a of a 16-k group consumes, in lane slot t, k = {0,3,12,15}[t] ^ {0,1,4,5}[a] (conflict-free).
+    int real_a_off[4], real_b_off[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        const int kl = (3 * (t & 1) + 12 * (t >> 1)) ^ ((a & 1) | ((a & 2) << 1));
+        real_a_off[a] = kl * 128 + (((g >> 1) ^ (kl & 7)) << 4) + ((g & 1) << 3);     // row ml = g; ml = g+8: ^ 64
+        real_b_off[a] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4) + ((kl & 1) << 3);
+    }
+
+    for (int kt = 0; kt < KT; ++kt) {
+        const int s = kt % STAGES;
+        mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
+        const unsigned char *sa = smem + s * S::STAGE_BYTES;
+        const unsigned char *sb = sa + S::A_BYTES;
+
+        if (CPLX) {
+            // 128B row = 8 complex.  A row index = mg*BK + k (mg = 8-row group), chunk = m ^ (k&7).
+            //                        B row index = kg*BN + n (kg = 8-k group),  chunk = (k&7) ^ (n&7).
+#pragma unroll
+            for (int kq = 0; kq < BK / 8; ++kq) {
+#pragma unroll
+                for (int a = 0; a < 2; ++a) {
+                    const int k7 = 2 * t + a;            // k & 7 of this lane's slot
+                    const int k = kq * 8 + k7;
+                    double ar[MB], ai[MB], nai[MB];
+#pragma unroll
+                    for (int i = 0; i < MB; ++i) {
+                        const int mg = wm * (C::WM / 8) + i;
+                        const double2 v = *reinterpret_cast<const double2 *>(
+                            sa + (mg * BK + k) * 128 + ((g ^ k7) << 4));
+                        ar[i] = v.x; ai[i] = v.y; nai[i] = -v.y;
+                    }
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        if (!FULL && j >= jmax) break;
+                        const int n = (j * WARPS_N + wn) * 8 + g;
+                        const double2 b = *reinterpret_cast<const double2 *>(
+                            sb + (kq * BN + n) * 128 + ((k7 ^ g) << 4));
+#pragma unroll
+                        for (int i = 0; i < MB; ++i) {
+                            dmma884(acc[0][i][j][0], acc[0][i][j][1], ar[i], b.x);    // Cr += Ar Br
+                            dmma884(acc[0][i][j][0], acc[0][i][j][1], nai[i], b.y);   // Cr -= Ai Bi
+                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ar[i], b.y);    // Ci += Ar Bi
+                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ai[i], b.x);    // Ci += Ai Br
+                        }
+                    }
+                }
+            }
+        } else {
+            // 128B row = 16 doubles.  A row index = mg*BK + k (mg = 16-row group), chunk = (m>>1) ^ (k&7);
+            //                         B row index = kg*BN + n (kg = 16-k group),   chunk = (k>>1) ^ (n&7).
+#pragma unroll
+            for (int kq = 0; kq < BK / 16; ++kq) {
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    double af[MB];
+#pragma unroll
+                    for (int i = 0; i < MB; ++i) {
+                        const int mg = wm * (C::WM / 16) + (i >> 1);
+                        af[i] = *reinterpret_cast<const double *>(
+                            sa + (mg * BK + kq * 16) * 128 + (real_a_off[a] ^ ((i & 1) << 6)));
+                    }
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        if (!FULL && j >= jmax) break;
+                        const double b = *reinterpret_cast<const double *>(
+                            sb + (kq * BN + (j * WARPS_N + wn) * 8) * 128 + real_b_off[a]);
+#pragma unroll
+                        for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+    }
+
+}
+
 template <bool CPLX>
 __global__ void __launch_bounds__(kThreads, 1)
 step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
@@ -141,9 +242,26 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     const uint32_t bar_base = smem_base + STAGES * S::STAGE_BYTES;   // full[STAGES], empty[STAGES]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int tile_m, tile_n;
-    tile_coords<C::GROUP_N>(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
-    const int m0 = tile_m * BM, n0 = tile_n * BN;
+    // Column tiling (DESIGN.md 6.1 "ragged and narrow tiles"): tiles_wide tiles of BN columns first,
+    // then tiles_narrow tiles of narrow_w columns (launched last, so that the tail of the launch is
+    // made of short CTAs).  A tile with `ncols_tile` valid columns only computes its first
+    // ceil(ncols_tile / 8) 8-column MMA blocks; block nb belongs to warp column nb % WARPS_N, so the
+    // remaining work stays balanced over the warps and the tile's time is ~ ceil(nblk / WARPS_N).
+    int tile_m, tile_n, n0, ncols_tile;
+    {
+        const int wide_ctas = p.tiles_m * p.tiles_wide;
+        if ((int)blockIdx.x < wide_ctas) {
+            tile_coords<C::GROUP_N>(blockIdx.x, p.tiles_m, p.tiles_wide, tile_m, tile_n);
+            n0 = tile_n * BN;
+            ncols_tile = min(BN, p.n - n0);
+        } else {
+            tile_coords<C::GROUP_N>(blockIdx.x - wide_ctas, p.tiles_m, p.tiles_narrow, tile_m, tile_n);
+            n0 = p.tiles_wide * BN + tile_n * p.narrow_w;
+            ncols_tile = min(p.narrow_w, p.n - n0);
+        }
+    }
+    const int m0 = tile_m * BM;
+    const int nblk = (ncols_tile + 7) >> 3;
     const int KT = (int)((p.N + BK - 1) / BK);
 
     if (threadIdx.x == 0) {
@@ -186,7 +304,10 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     // ---------------------------------------------------------------- consumer warps
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
     const int g = lane >> 2, t = lane & 3;
+    constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
+    static_assert(WARPS_N * C::WN == BN, "warp grid must cover the CTA tile");
     const int wm = warp % C::WARPS_M, wn = warp / C::WARPS_M;
+    const int jmax = (nblk - wn + WARPS_N - 1) / WARPS_N;    // this warp owns blocks nb = j * WARPS_N + wn, j < jmax
 
     double acc[CPLX ? 2 : 1][MB][NB][2];
 #pragma unroll
@@ -196,81 +317,8 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 #pragma unroll
             for (int j = 0; j < NB; ++j) acc[q][i][j][0] = acc[q][i][j][1] = 0.0;
 
-    // float64: lane-dependent byte offsets of the fragment loads, hoisted out of the k loop.
-    // MMA a of a 16-k group consumes, in lane slot t, k = {0,3,12,15}[t] ^ {0,1,4,5}[a] (conflict-free).
-    int real_a_off[4], real_b_off[4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-        const int kl = (3 * (t & 1) + 12 * (t >> 1)) ^ ((a & 1) | ((a & 2) << 1));
-        real_a_off[a] = kl * 128 + (((g >> 1) ^ (kl & 7)) << 4) + ((g & 1) << 3);     // row ml = g; ml = g+8: ^ 64
-        real_b_off[a] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4) + ((kl & 1) << 3);
-    }
-
-    for (int kt = 0; kt < KT; ++kt) {
-        const int s = kt % STAGES;
-        mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
-        const unsigned char *sa = smem + s * S::STAGE_BYTES;
-        const unsigned char *sb = sa + S::A_BYTES;
-
-        if (CPLX) {
-            // 128B row = 8 complex.  A row index = mg*BK + k (mg = 8-row group), chunk = m ^ (k&7).
-            //                        B row index = kg*BN + n (kg = 8-k group),  chunk = (k&7) ^ (n&7).
-#pragma unroll
-            for (int kq = 0; kq < BK / 8; ++kq) {
-#pragma unroll
-                for (int a = 0; a < 2; ++a) {
-                    const int k7 = 2 * t + a;            // k & 7 of this lane's slot
-                    const int k = kq * 8 + k7;
-                    double ar[MB], ai[MB], nai[MB];
-#pragma unroll
-                    for (int i = 0; i < MB; ++i) {
-                        const int mg = wm * (C::WM / 8) + i;
-                        const double2 v = *reinterpret_cast<const double2 *>(
-                            sa + (mg * BK + k) * 128 + ((g ^ k7) << 4));
-                        ar[i] = v.x; ai[i] = v.y; nai[i] = -v.y;
-                    }
-#pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        const int n = wn * C::WN + j * 8 + g;
-                        const double2 b = *reinterpret_cast<const double2 *>(
-                            sb + (kq * BN + n) * 128 + ((k7 ^ g) << 4));
-#pragma unroll
-                        for (int i = 0; i < MB; ++i) {
-                            dmma884(acc[0][i][j][0], acc[0][i][j][1], ar[i], b.x);    // Cr += Ar Br
-                            dmma884(acc[0][i][j][0], acc[0][i][j][1], nai[i], b.y);   // Cr -= Ai Bi
-                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ar[i], b.y);    // Ci += Ar Bi
-                            dmma884(acc[1][i][j][0], acc[1][i][j][1], ai[i], b.x);    // Ci += Ai Br
-                        }
-                    }
-                }
-            }
-        } else {
-            // 128B row = 16 doubles.  A row index = mg*BK + k (mg = 16-row group), chunk = (m>>1) ^ (k&7);
-            //                         B row index = kg*BN + n (kg = 16-k group),   chunk = (k>>1) ^ (n&7).
-#pragma unroll
-            for (int kq = 0; kq < BK / 16; ++kq) {
-#pragma unroll
-                for (int a = 0; a < 4; ++a) {
-                    double af[MB];
-#pragma unroll
-                    for (int i = 0; i < MB; ++i) {
-                        const int mg = wm * (C::WM / 16) + (i >> 1);
-                        af[i] = *reinterpret_cast<const double *>(
-                            sa + (mg * BK + kq * 16) * 128 + (real_a_off[a] ^ ((i & 1) << 6)));
-                    }
-#pragma unroll
-                    for (int j = 0; j < NB; ++j) {
-                        const double b = *reinterpret_cast<const double *>(
-                            sb + (kq * BN + wn * C::WN + j * 8) * 128 + real_b_off[a]);
-#pragma unroll
-                        for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
-                    }
-                }
-            }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
-    }
+    if (jmax == NB) mainloop<CPLX, true>(acc, smem, bar_base, KT, lane, warp, jmax);
+    else mainloop<CPLX, false>(acc, smem, bar_base, KT, lane, warp, jmax);
 
     // ---------------------------------------------------------------- fused epilogue
     // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
@@ -280,8 +328,9 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     for (int j = 0; j < NB; ++j) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-            const int col = n0 + wn * C::WN + j * 8 + 2 * t + e;
-            if (col >= p.n) continue;
+            const int cl = (j * WARPS_N + wn) * 8 + 2 * t + e;     // column inside the tile
+            if (cl >= ncols_tile) continue;
+            const int col = n0 + cl;
             const double c = p.c_col ? p.c_col[col] : p.c;
 #pragma unroll
             for (int i = 0; i < MB; ++i) {
@@ -330,6 +379,18 @@ EncodeTiledFn get_encode_fn() {
     return fn;
 }
 
+int sm_count() {
+    static int sms = 0;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    });
+    return sms;
+}
+
 template <bool CPLX>
 cudaError_t encode_maps(DmmaPlan *plan) {
     using C = Cfg<CPLX>;
@@ -359,6 +420,70 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     return cudaSuccess;
 }
 
+// Time of one launch in units of a "quarter" tile (8 * WARPS_N columns x BM rows over all of k) on `sms`
+// SMs, one CTA per SM, CTAs dispatched in blockIdx order to the SM that frees first: `wide` CTAs of
+// `wide_cost` quarters, then `narrow` CTAs of `narrow_cost`.  SM loads are kept as (load, count) levels.
+struct Level { double load; int count; };
+void assign(std::vector<Level> &lv, int64_t T, double cost) {
+    while (T > 0) {
+        if (lv.size() == 1 && T >= lv[0].count) {          // whole rounds at once
+            const int64_t rounds = T / lv[0].count;
+            lv[0].load += (double)rounds * cost;
+            T -= rounds * lv[0].count;
+            continue;
+        }
+        const Level lo = lv.front();                          // levels are sorted by ascending load
+        const int m = (int)std::min<int64_t>(lo.count, T);
+        lv.front().count -= m;
+        if (lv.front().count == 0) lv.erase(lv.begin());
+        const double nl = lo.load + cost;
+        size_t i = 0;
+        while (i < lv.size() && lv[i].load < nl - 1e-9) ++i;
+        if (i < lv.size() && std::fabs(lv[i].load - nl) <= 1e-9) lv[i].count += m;
+        else lv.insert(lv.begin() + i, Level{nl, m});
+        T -= m;
+    }
+}
+double makespan(int sms, int64_t wide, double wide_cost, int64_t narrow, double narrow_cost) {
+    std::vector<Level> lv{Level{0.0, sms}};
+    assign(lv, wide, wide_cost);
+    assign(lv, narrow, narrow_cost);
+    return lv.back().load;
+}
+
+// Chooses the column tiling of one launch: `wide` tiles of BN columns, then tiles of `narrow_w` columns
+// (a multiple of the quarter width Q = 8 * WARPS_N) over the rest, minimising the modelled makespan.
+template <bool CPLX>
+void choose_tiling(int64_t n, int tiles_m, int sms, int &tiles_wide, int &tiles_narrow, int &narrow_w) {
+    using C = Cfg<CPLX>;
+    constexpr int Q = 8 * (kConsumerWarps / C::WARPS_M);      // columns per quarter tile
+    constexpr int QPT = C::BN / Q;                            // quarters per full tile (4)
+    constexpr double kNarrowOverhead = 0.06;                  // per-CTA cost of a narrow tile beyond its quarters
+    const int full_tiles = (int)(n / C::BN);
+    double best = 1e300;
+    tiles_wide = full_tiles; tiles_narrow = 0; narrow_w = C::BN;
+    const int backs[4] = {0, 1, 2, full_tiles};                         // full tiles handed to the narrow region
+    for (int bi = 0; bi < 4; ++bi) {
+        const int back = backs[bi];
+        if (back > full_tiles || (bi == 3 && back <= 2)) continue;
+        const int wide = full_tiles - back;
+        const int64_t rest = n - (int64_t)wide * C::BN;
+        if (rest == 0) {
+            const double t = makespan(sms, (int64_t)wide * tiles_m, QPT, 0, 0.0);
+            if (t < best) { best = t; tiles_wide = wide; tiles_narrow = 0; narrow_w = C::BN; }
+            continue;
+        }
+        for (int wq = 1; wq <= QPT; ++wq) {
+            const int w = wq * Q;
+            const int64_t nt = (rest + w - 1) / w;
+            // cost of the narrow tiles: all but the last have wq quarters; model the last one the same
+            const double t = makespan(sms, (int64_t)wide * tiles_m, QPT, nt * tiles_m, wq + kNarrowOverhead);
+            // total work also matters when the launch is shorter than one wave: prefer fewer, wider tiles on ties
+            if (t < best - 1e-9) { best = t; tiles_wide = wide; tiles_narrow = (int)nt; narrow_w = w; }
+        }
+    }
+}
+
 template <bool CPLX>
 cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
                    cudaStream_t stream, const double *c_col) {
@@ -380,7 +505,7 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     p.n = (int)n;
     p.col0 = (int)s;
     p.tiles_m = (int)((plan->N + C::BM - 1) / C::BM);
-    p.tiles_n = (int)((n + C::BN - 1) / C::BN);
+    choose_tiling<CPLX>(n, p.tiles_m, sm_count(), p.tiles_wide, p.tiles_narrow, p.narrow_w);
     p.alpha = alpha;
     p.beta = beta;
     p.c = c;
@@ -388,12 +513,20 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     p.use_beta = use_beta;
     const CUtensorMap *mA = (const CUtensorMap *)plan->tmap_H;
     const CUtensorMap *mB = (const CUtensorMap *)plan->tmap_B[src];
-    step_dmma_kernel<CPLX><<<(unsigned)(p.tiles_m * p.tiles_n), kThreads, Smem<CPLX>::TOTAL, stream>>>(*mA, *mB, p);
+    step_dmma_kernel<CPLX><<<(unsigned)(p.tiles_m * (p.tiles_wide + p.tiles_narrow)), kThreads, Smem<CPLX>::TOTAL, stream>>>(*mA, *mB, p);
     count_launch();
     return cudaGetLastError();
 }
 
 }  // namespace
+
+void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_t out[4]) {
+    int tw = 0, tn = 0, nw = 0;
+    const int tiles_m = (int)((N + 127) / 128);
+    if (dtype == CHASE_C128) choose_tiling<true>(n, tiles_m, sms, tw, tn, nw);
+    else choose_tiling<false>(n, tiles_m, sms, tw, tn, nw);
+    out[0] = tiles_m; out[1] = tw; out[2] = tn; out[3] = nw;
+}
 
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     if (ncols < 1 || N < 16 || N > (1 << 28) || ncols > (1 << 28)) return false;

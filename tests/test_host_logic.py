@@ -7,6 +7,7 @@ import re
 
 import numpy as np
 import pytest
+import torch
 
 import oracle
 import paper_1805_10121_b200 as pkg
@@ -123,3 +124,24 @@ def test_product_does_not_import_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1805_10121_b200" not in src and "from paper_1805_10121_b200" not in src, f
             assert "#include \"chase" not in src, f
+
+
+@pytest.mark.parametrize("dtype,bn,quarter", [(torch.complex128, 64, 16), (torch.float64, 128, 32)])
+def test_step_tiling_covers_every_column_once(dtype, bn, quarter):
+    """chase_filter_step_tiling: wide tiles then narrow tiles cover [0, n) exactly; the narrow width is a
+    multiple of the quarter width; never more narrow columns than needed (host model only, no CUDA)."""
+    for N in (512, 4096, 40000):
+        for n in list(range(1, 200)) + [255, 256, 257, 1400, 1867, 2000, 2999]:
+            for sms in (148, 132):
+                tm, tw, tn, nw = pkg.chase_filter_step_tiling(N, n, dtype, sms)
+                assert tm == -(-N // 128)
+                assert 0 <= tw * bn <= n
+                rest = n - tw * bn
+                assert nw % quarter == 0 and quarter <= nw <= bn
+                assert tn == -(-rest // nw), (N, n, tw, tn, nw)
+
+
+def test_step_tiling_shortens_the_tail_of_the_metric_config():
+    """cfg 4 full width: 2000 = 31 x 64 + 16 columns; the ragged 16 columns must not cost a full tile."""
+    tm, tw, tn, nw = pkg.chase_filter_step_tiling(40000, 2000, torch.complex128, 148)
+    assert (tm, tw) == (313, 31) and tn * nw >= 16 and nw < 64
