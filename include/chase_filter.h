@@ -140,6 +140,34 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
                     double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
                     void *stream);
 
+/* Spectral estimates (Alg. 6 "Lanczos procedure for parameters estimates",
+ * PAPER.md:421-475; Eq. (9)-(10)).
+ *
+ * chase_lanczos: `nruns` independent Lanczos runs of k steps each, advanced together so that the
+ *   matrix-vector products of one step are ONE HEMM on an N x nruns block.  Run r
+ *   starts from column r of V0 (DEVICE, N x nruns column-major, read only; the method's random start
+ *   vectors are the caller's, they need not be normalised).  Every new Lanczos vector is
+ *   re-orthogonalised against all previous ones of its run (two classical Gram-Schmidt passes).
+ *   Output (HOST): alpha[r * k + j], beta[r * k + j], j = 0..k-1, with
+ *       A U = U T_k + f_k e_k^T,  T_k = tridiag(beta[0..k-2]; alpha[0..k-1]; beta[0..k-2]),  beta[k-1] = ||f_k||_2.
+ *   k <= N.  workspace DEVICE >= chase_lanczos_workspace_bytes(...), 16-byte aligned.  Enqueues on
+ *   `stream` and SYNCHRONISES it before returning (the outputs are host arrays).
+ *
+ * chase_spectral_estimates (host only): from the coefficients of nruns = 1 + n_vec runs,
+ *       b_sup = ||f_k||_2 + max Ritz value of run 0                                   (Alg. 6 l.3)
+ *       mu_1  = smallest Ritz value over runs 1..n_vec                                (l.12)
+ *       mu_ne = t with  int_{-inf}^{t} phi~ = nev_nex / N,                            (l.10-11)
+ *       phi~(t) = 1/n_vec sum_j sum_i (Z^[j]_{1,i})^2 g_sigma(t - lambda~^[j]_i)      (Eq. 10)
+ *   with g_sigma the Gaussian density of standard deviation sigma (paper default 0.25).
+ *   nruns == 1 is the `approx` branch (l.4-5): only *b_sup is written (mu_1, mu_ne may be NULL).
+ *   nev_nex is a double so that callers can aim between two eigenvalues; 0 < nev_nex < N.
+ *   Returns 0 or CHASE_ERR_ARG (null pointer, bad size, non-finite / negative coefficient, sigma <= 0). */
+size_t chase_lanczos_workspace_bytes(int64_t N, int64_t nruns, int32_t k, chase_dtype_t dtype);
+int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nruns, int32_t k, chase_dtype_t dtype,
+                  double *alpha, double *beta, void *workspace, size_t workspace_bytes, void *stream);
+int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, const double *beta, int64_t N,
+                             double nev_nex, double sigma, double *b_sup, double *mu_1, double *mu_ne);
+
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
  * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
  * N % 4 == 0; needs the larger workspace chase_filter_workspace_bytes reports), 0 = generic FMA

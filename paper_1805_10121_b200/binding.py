@@ -22,6 +22,7 @@ EXPORTS = [
     "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
     "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_tiling",
+    "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates",
 ]
 
 _lib = None
@@ -77,6 +78,12 @@ def load() -> ctypes.CDLL:
     lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
     lib.chase_filter_step_tiling.restype = ctypes.c_int
     lib.chase_filter_step_tiling.argtypes = [i64, i64, ctypes.c_int, i32, vp]
+    lib.chase_lanczos_workspace_bytes.restype = sz
+    lib.chase_lanczos_workspace_bytes.argtypes = [i64, i64, i32, ctypes.c_int]
+    lib.chase_lanczos.restype = ctypes.c_int
+    lib.chase_lanczos.argtypes = [vp, i64, vp, i64, i32, ctypes.c_int, vp, vp, vp, sz, vp]
+    lib.chase_spectral_estimates.restype = ctypes.c_int
+    lib.chase_spectral_estimates.argtypes = [i32, i64, vp, vp, i64, dbl, dbl, vp, vp, vp]
     lib.chase_filter_strerror.restype = ctypes.c_char_p
     lib.chase_filter_strerror.argtypes = [ctypes.c_int]
     _lib = lib
@@ -284,3 +291,47 @@ def chase_residuals(H: torch.Tensor, V: torch.Tensor, ritzv, workspace: Optional
                                       _DTYPE_CODE[H.dtype], workspace.data_ptr(),
                                       workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
     return resid
+
+
+def chase_lanczos_workspace_bytes(N: int, nruns: int, k: int, dtype: torch.dtype) -> int:
+    return int(load().chase_lanczos_workspace_bytes(N, nruns, k, _DTYPE_CODE[dtype]))
+
+
+def chase_lanczos(H: torch.Tensor, V0: torch.Tensor, k: int, workspace: Optional[torch.Tensor] = None,
+                  stream: Optional[torch.cuda.Stream] = None):
+    """k Lanczos steps for every column of V0 (Alg. 6 l.2 / l.8), coalesced into one HEMM per step.
+    Returns host arrays (alpha[nruns, k], beta[nruns, k]); synchronises the stream."""
+    if not (H.is_cuda and V0.is_cuda):
+        raise ValueError("H and V0 must be CUDA tensors (there is no CPU path)")
+    if H.dtype != V0.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V0 must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V0, "V0")
+    N, nruns = V0.shape
+    if H.shape != (N, N):
+        raise ValueError("shape mismatch")
+    need = chase_lanczos_workspace_bytes(N, nruns, k, H.dtype)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), dtype=torch.uint8, device=H.device)
+    alpha = np.zeros((nruns, k), dtype=np.float64)
+    beta = np.zeros((nruns, k), dtype=np.float64)
+    with torch.cuda.device(H.device):
+        _check(load().chase_lanczos(H.data_ptr(), N, V0.data_ptr(), nruns, int(k), _DTYPE_CODE[H.dtype],
+                                    alpha.ctypes.data, beta.ctypes.data, workspace.data_ptr(),
+                                    workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return alpha, beta
+
+
+def chase_spectral_estimates(alpha, beta, N: int, nev_nex: float, sigma: float = 0.25):
+    """(b_sup, mu_1, mu_nev_nex) of Alg. 6 from the coefficients of 1 + n_vec Lanczos runs (host only);
+    a single run gives (b_sup, None, None)."""
+    a = np.ascontiguousarray(np.asarray(alpha, dtype=np.float64))
+    b = np.ascontiguousarray(np.asarray(beta, dtype=np.float64))
+    if a.ndim != 2 or a.shape != b.shape:
+        raise ValueError("alpha and beta must be [nruns, k] arrays of equal shape")
+    nruns, k = a.shape
+    out = (ctypes.c_double * 3)()
+    base = ctypes.addressof(out)
+    _check(load().chase_spectral_estimates(int(k), int(nruns), a.ctypes.data, b.ctypes.data, int(N), float(nev_nex),
+                                           float(sigma), base, base + 8, base + 16))
+    return (out[0], None, None) if nruns == 1 else (out[0], out[1], out[2])

@@ -133,8 +133,11 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
     return CHASE_OK;
 }
 
+}  // extern "C"
+
 // One launch of the step kernel family: Y <- alpha (H X - c X) + beta Y with X, Y whole buffers.
-static int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha,
+namespace chase {
+int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha,
                            double beta, double c, const double *c_col, int use_beta, chase_dtype_t dtype,
                            cudaStream_t stream) {
     if (chase_filter_kernel_path(N, ncols, dtype) == 1) {
@@ -149,6 +152,9 @@ static int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int
     sa.alpha = alpha; sa.beta = beta; sa.c = c; sa.c_col = c_col; sa.use_beta = use_beta;
     return (int)launch_step_generic(dtype, sa, stream);
 }
+}  // namespace chase
+
+extern "C" {
 
 int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
                double alpha, double beta, double shift, chase_dtype_t dtype, void *stream_) {
@@ -190,6 +196,65 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
     int rc = launch_one_step(H, N, V, workspace, ncols, 1.0, 0.0, 0.0, d_shift, 0, dtype, stream);
     if (rc != CHASE_OK) return rc;
     return (int)launch_column_norms(dtype, workspace, N, ncols, resid, stream);
+}
+
+size_t chase_lanczos_workspace_bytes(int64_t N, int64_t nvec, int32_t k, chase_dtype_t dtype) {
+    const size_t w = elem_bytes(dtype);
+    if (w == 0 || N <= 0 || nvec <= 0 || k <= 0 || N > kMaxDim || nvec > 4096 || k > 4096 || k > N) return 0;
+    return lanczos_workspace_bytes(N, nvec, k, w);
+}
+
+int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nvec, int32_t k, chase_dtype_t dtype,
+                  double *alpha, double *beta, void *workspace, size_t workspace_bytes, void *stream_) {
+    const size_t w = elem_bytes(dtype);
+    if (w == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || nvec <= 0 || k <= 0 || N > kMaxDim || nvec > 4096 || k > 4096 || k > N) return CHASE_ERR_ARG;
+    if (!H || !V0 || !alpha || !beta) return CHASE_ERR_ARG;
+    if (!workspace || workspace_bytes < lanczos_workspace_bytes(N, nvec, k, w)) return CHASE_ERR_WORKSPACE;
+    if (((uintptr_t)H | (uintptr_t)V0 | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
+    return (int)lanczos_run(H, N, V0, (int)nvec, k, dtype, w, workspace, alpha, beta, (cudaStream_t)stream_);
+}
+
+int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, const double *beta, int64_t N,
+                             double nev_nex, double sigma, double *b_sup, double *mu_1, double *mu_ne) {
+    if (k <= 0 || nruns <= 0 || !alpha || !beta || !b_sup || N <= 0) return CHASE_ERR_ARG;
+    for (int64_t i = 0; i < nruns * k; ++i)
+        if (!std::isfinite(alpha[i]) || !std::isfinite(beta[i]) || beta[i] < 0.0) return CHASE_ERR_ARG;
+    std::vector<double> lam, wt;
+    if (!lanczos_ritz(k, alpha, beta, lam, wt)) return CHASE_ERR_ARG;
+    *b_sup = beta[k - 1] + *std::max_element(lam.begin(), lam.end());          // Alg. 6 l.3
+    if (nruns == 1) return CHASE_OK;                                            // l.4-5 (`approx`)
+    if (!mu_1 || !mu_ne || !(sigma > 0.0) || !std::isfinite(sigma) || !(nev_nex > 0.0) || !(nev_nex < (double)N))
+        return CHASE_ERR_ARG;
+    std::vector<double> lams, wts;                                              // l.7-8: runs 1 .. n_vec
+    double lo = 0.0, hi = 0.0, mu1 = 0.0;
+    for (int64_t r = 1; r < nruns; ++r) {
+        if (!lanczos_ritz(k, alpha + r * k, beta + r * k, lam, wt)) return CHASE_ERR_ARG;
+        const double mn = *std::min_element(lam.begin(), lam.end()), mx = *std::max_element(lam.begin(), lam.end());
+        if (r == 1 || mn < mu1) mu1 = mn;                                       // l.12
+        if (r == 1 || mn < lo) lo = mn;
+        if (r == 1 || mx > hi) hi = mx;
+        lams.insert(lams.end(), lam.begin(), lam.end());
+        wts.insert(wts.end(), wt.begin(), wt.end());
+    }
+    // l.10-11: the integral of phi~ (Eq. 10) up to t is sum_j w_j Phi((t - lam_j) / sigma) / n_vec; it is
+    // strictly increasing in t, so the root is found by bisection.
+    const double target = nev_nex / (double)N, inv = 1.0 / (sigma * std::sqrt(2.0)), nv = (double)(nruns - 1);
+    auto integral = [&](double t) {
+        double s = 0.0;
+        for (size_t i = 0; i < lams.size(); ++i) s += wts[i] * 0.5 * std::erfc(-(t - lams[i]) * inv);
+        return s / nv;
+    };
+    lo -= 40.0 * sigma;
+    hi += 40.0 * sigma;
+    for (int it = 0; it < 300 && hi - lo > 0.0; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (mid <= lo || mid >= hi) break;
+        if (integral(mid) < target) lo = mid; else hi = mid;
+    }
+    *mu_ne = 0.5 * (lo + hi);
+    *mu_1 = mu1;
+    return CHASE_OK;
 }
 
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {

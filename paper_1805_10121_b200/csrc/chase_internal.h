@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <vector>
 #include "chase_filter.h"
 
 namespace chase {
@@ -67,6 +68,19 @@ cudaError_t tf32_launch_step(const Tf32Plan *plan, int src, int64_t s, double al
 // resid[j] = || R[:, j] ||_2 for an N x n column-major block R (device), resid device double[n].
 cudaError_t launch_column_norms(chase_dtype_t dtype, const void *R, int64_t N, int64_t n, double *resid,
                                 cudaStream_t stream);
+
+// One launch of the step kernel family on whole buffers: Y <- alpha (H X - c X) + beta Y (c_col: optional
+// per-column shift).  Returns 0, a negative CHASE_ERR_* or a positive cudaError_t.
+int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha, double beta,
+                    double c, const double *c_col, int use_beta, chase_dtype_t dtype, cudaStream_t stream);
+
+// Alg. 6: 1 + n_vec coalesced Lanczos runs (csrc/lanczos.cu).  alpha_host / beta_host: HOST [nvec * k],
+// run r at offset r * k.  Synchronises `stream`.
+size_t lanczos_workspace_bytes(int64_t N, int64_t nvec, int32_t k, size_t elem);
+cudaError_t lanczos_run(const void *H, int64_t N, const void *V0, int nvec, int k, chase_dtype_t dtype, size_t elem,
+                        void *workspace, double *alpha_host, double *beta_host, cudaStream_t stream);
+// Ritz values (unsorted) and squared first eigenvector components of T_k; false = QL did not converge.
+bool lanczos_ritz(int k, const double *alpha, const double *beta, std::vector<double> &lam, std::vector<double> &w);
 
 void count_launch();
 

@@ -1,0 +1,249 @@
+// Spectral estimates (Alg. 6 "Lanczos procedure for parameters estimates", PAPER.md:421-475;
+// Eq. (9)-(10)): 1 + n_vec Lanczos runs of k steps advanced TOGETHER, so that the
+// matrix-vector products of one step are a single HEMM on an N x (1 + n_vec) block ("the n_vec
+// matrix-vector multiplications are coalesced into a single HEMM") -- the step kernel
+// of the filter with alpha = 1, beta = 0, no shift.  Everything else of a step (Gram-Schmidt
+// coefficients, vector updates, norms) runs in the small kernels below without leaving the device;
+// the 2 k (1 + n_vec) Lanczos coefficients are copied to the host once at the end, where the
+// tridiagonal eigenproblems, the DoS integral and b_sup are evaluated (chase_spectral_estimates).
+//
+// Reading G19: full re-orthogonalisation by two passes of classical Gram-Schmidt against
+// all previous Lanczos vectors; alpha_j is the j-th coefficient of the first pass.
+#include <cmath>
+#include <vector>
+
+#include "chase_internal.h"
+
+namespace chase {
+namespace {
+
+constexpr int kBlock = 256;
+
+template <typename T> struct Elem;
+template <> struct Elem<float>   { using real = float;  static constexpr bool cplx = false; };
+template <> struct Elem<double>  { using real = double; static constexpr bool cplx = false; };
+template <> struct Elem<float2>  { using real = float;  static constexpr bool cplx = true; };
+template <> struct Elem<double2> { using real = double; static constexpr bool cplx = true; };
+
+__device__ __forceinline__ double2 ld(const float *p, int64_t i)   { return make_double2((double)p[i], 0.0); }
+__device__ __forceinline__ double2 ld(const double *p, int64_t i)  { return make_double2(p[i], 0.0); }
+__device__ __forceinline__ double2 ld(const float2 *p, int64_t i)  { const float2 v = p[i]; return make_double2(v.x, v.y); }
+__device__ __forceinline__ double2 ld(const double2 *p, int64_t i) { return p[i]; }
+__device__ __forceinline__ void st(float *p, int64_t i, double2 v)   { p[i] = (float)v.x; }
+__device__ __forceinline__ void st(double *p, int64_t i, double2 v)  { p[i] = v.x; }
+__device__ __forceinline__ void st(float2 *p, int64_t i, double2 v)  { p[i] = make_float2((float)v.x, (float)v.y); }
+__device__ __forceinline__ void st(double2 *p, int64_t i, double2 v) { p[i] = v; }
+
+// Sum of a double2 over the block; result valid in thread 0.
+__device__ __forceinline__ double2 block_sum(double2 v) {
+    __shared__ double2 part[kBlock / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        v.x += __shfl_down_sync(0xffffffffu, v.x, o);
+        v.y += __shfl_down_sync(0xffffffffu, v.y, o);
+    }
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = threadIdx.x < kBlock / 32 ? part[threadIdx.x] : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            v.x += __shfl_down_sync(0xffffffffu, v.x, o);
+            v.y += __shfl_down_sync(0xffffffffu, v.y, o);
+        }
+    }
+    return v;
+}
+
+// h[i, c] = U_i[:, c]^H w[:, c]  for i = blockIdx.x <= j, run c = blockIdx.y.  U_i is block i of U
+// (each block N x nvec, column-major).  pass 0 also records alpha_j[c] = Re h[j, c].
+template <typename T>
+__global__ void __launch_bounds__(kBlock) lz_project(const T *__restrict__ U, const T *__restrict__ w, int64_t N,
+                                                     int nvec, int j, double2 *__restrict__ h,
+                                                     double *__restrict__ alpha, int k, int pass) {
+    const int i = blockIdx.x, c = blockIdx.y;
+    const T *u = U + ((int64_t)i * nvec + c) * N;
+    const T *x = w + (int64_t)c * N;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int64_t r = threadIdx.x; r < N; r += kBlock) {
+        const double2 a = ld(u, r), b = ld(x, r);
+        acc.x += a.x * b.x + a.y * b.y;          // conj(a) * b
+        acc.y += a.x * b.y - a.y * b.x;
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) {
+        h[(int64_t)i * nvec + c] = acc;
+        if (pass == 0 && i == j) alpha[(int64_t)c * k + j] = acc.x;
+    }
+}
+
+// w[:, c] -= sum_{i <= j} h[i, c] U_i[:, c]
+template <typename T>
+__global__ void __launch_bounds__(kBlock) lz_update(const T *__restrict__ U, T *__restrict__ w, int64_t N, int nvec,
+                                                    int j, const double2 *__restrict__ h) {
+    const int c = blockIdx.y;
+    const int64_t r = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (r >= N) return;
+    T *x = w + (int64_t)c * N;
+    double2 v = ld(x, r);
+    for (int i = 0; i <= j; ++i) {
+        const double2 a = ld(U + ((int64_t)i * nvec + c) * N, r);
+        const double2 g = h[(int64_t)i * nvec + c];
+        v.x -= g.x * a.x - g.y * a.y;
+        v.y -= g.x * a.y + g.y * a.x;
+    }
+    st(x, r, v);
+}
+
+// out[c * stride + idx] = || x[:, c] ||_2
+template <typename T>
+__global__ void __launch_bounds__(kBlock) lz_colnorm(const T *__restrict__ x, int64_t N, double *__restrict__ out,
+                                                     int stride, int idx) {
+    const int c = blockIdx.x;
+    const T *p = x + (int64_t)c * N;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int64_t r = threadIdx.x; r < N; r += kBlock) {
+        const double2 a = ld(p, r);
+        acc.x += a.x * a.x + a.y * a.y;
+    }
+    acc = block_sum(acc);
+    if (threadIdx.x == 0) out[(int64_t)c * stride + idx] = sqrt(acc.x);
+}
+
+// y[:, c] = x[:, c] / nrm[c * stride + idx]
+template <typename T>
+__global__ void __launch_bounds__(kBlock) lz_scale(const T *__restrict__ x, T *__restrict__ y, int64_t N,
+                                                   const double *__restrict__ nrm, int stride, int idx) {
+    const int c = blockIdx.y;
+    const int64_t r = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (r >= N) return;
+    const double s = 1.0 / nrm[(int64_t)c * stride + idx];
+    const double2 v = ld(x + (int64_t)c * N, r);
+    st(y + (int64_t)c * N, r, make_double2(v.x * s, v.y * s));
+}
+
+size_t round256(size_t b) { return (b + 255) / 256 * 256; }
+
+template <typename T>
+cudaError_t run(const void *H, int64_t N, const void *V0, int nvec, int k, chase_dtype_t dtype, void *workspace,
+                double *d_alpha, double *d_beta, double2 *d_h, cudaStream_t stream) {
+    T *U = (T *)workspace;                                            // k blocks of N x nvec
+    T *w = U + (size_t)k * N * nvec;                                  // N x nvec
+    const dim3 grid_rows((unsigned)((N + kBlock - 1) / kBlock), (unsigned)nvec);
+    // u_0 = v_0 / ||v_0||; the start norm is parked in beta[.., 0] and overwritten by step 0
+    lz_colnorm<T><<<nvec, kBlock, 0, stream>>>((const T *)V0, N, d_beta, k, 0);
+    lz_scale<T><<<grid_rows, kBlock, 0, stream>>>((const T *)V0, U, N, d_beta, k, 0);
+    count_launch(); count_launch();
+    for (int j = 0; j < k; ++j) {
+        const T *uj = U + (size_t)j * N * nvec;
+        int rc = launch_one_step(H, N, uj, w, nvec, 1.0, 0.0, 0.0, nullptr, 0, dtype, stream);   // w = A u_j, all runs
+        if (rc != 0) return rc > 0 ? (cudaError_t)rc : cudaErrorInvalidValue;
+        for (int pass = 0; pass < 2; ++pass) {
+            lz_project<T><<<dim3(j + 1, nvec), kBlock, 0, stream>>>(U, w, N, nvec, j, d_h, d_alpha, k, pass);
+            lz_update<T><<<grid_rows, kBlock, 0, stream>>>(U, w, N, nvec, j, d_h);
+            count_launch(); count_launch();
+        }
+        lz_colnorm<T><<<nvec, kBlock, 0, stream>>>(w, N, d_beta, k, j);     // beta_j = ||w||; j = k-1: ||f_k||
+        count_launch();
+        if (j + 1 < k) {
+            lz_scale<T><<<grid_rows, kBlock, 0, stream>>>(w, U + (size_t)(j + 1) * N * nvec, N, d_beta, k, j);
+            count_launch();
+        }
+    }
+    return cudaGetLastError();
+}
+
+// Eigenvalues of the symmetric tridiagonal T (diagonal d[0..n), off-diagonal e[0..n-1)) and the FIRST
+// components of its normalised eigenvectors, by the implicit-shift QL iteration with the rotations
+// applied to the row vector z = e_1^T only (Golub-Welsch).  On return d holds the eigenvalues
+// (unsorted), z the first components.  Returns false if an eigenvalue needs more than 60 sweeps.
+bool tridiag_ql_first_row(int n, std::vector<double> &d, std::vector<double> &e, std::vector<double> &z) {
+    e.resize(n, 0.0);
+    z.assign(n, 0.0);
+    z[0] = 1.0;
+    const double eps = 2.220446049250313e-16;
+    for (int l = 0; l < n; ++l) {
+        int iter = 0, m;
+        do {
+            for (m = l; m < n - 1; ++m) {
+                const double dd = std::fabs(d[m]) + std::fabs(d[m + 1]);
+                if (std::fabs(e[m]) <= eps * dd) break;
+            }
+            if (m != l) {
+                if (++iter > 60) return false;
+                double g = (d[l + 1] - d[l]) / (2.0 * e[l]);
+                double r = std::hypot(g, 1.0);
+                g = d[m] - d[l] + e[l] / (g + (g >= 0.0 ? std::fabs(r) : -std::fabs(r)));
+                double s = 1.0, c = 1.0, p = 0.0;
+                int i;
+                for (i = m - 1; i >= l; --i) {
+                    double f = s * e[i];
+                    const double b = c * e[i];
+                    r = std::hypot(f, g);
+                    e[i + 1] = r;
+                    if (r == 0.0) {
+                        d[i + 1] -= p;
+                        e[m] = 0.0;
+                        break;
+                    }
+                    s = f / r;
+                    c = g / r;
+                    g = d[i + 1] - p;
+                    r = (d[i] - g) * s + 2.0 * c * b;
+                    p = s * r;
+                    d[i + 1] = g + p;
+                    g = c * r - b;
+                    f = z[i + 1];
+                    z[i + 1] = s * z[i] + c * f;
+                    z[i] = c * z[i] - s * f;
+                }
+                if (r == 0.0 && i >= l) continue;
+                d[l] -= p;
+                e[l] = g;
+                e[m] = 0.0;
+            }
+        } while (m != l);
+    }
+    return true;
+}
+
+}  // namespace
+
+size_t lanczos_workspace_bytes(int64_t N, int64_t nvec, int32_t k, size_t elem) {
+    const size_t vec = (size_t)N * (size_t)nvec * elem;
+    return round256(vec * (size_t)k) + round256(vec)                      // U (k blocks), w
+           + 2 * round256((size_t)nvec * k * sizeof(double))              // alpha, beta
+           + round256((size_t)nvec * k * sizeof(double2));                // Gram-Schmidt coefficients
+}
+
+cudaError_t lanczos_run(const void *H, int64_t N, const void *V0, int nvec, int k, chase_dtype_t dtype, size_t elem,
+                        void *workspace, double *alpha_host, double *beta_host, cudaStream_t stream) {
+    const size_t vec = (size_t)N * (size_t)nvec * elem;
+    char *base = (char *)workspace;
+    double *d_alpha = (double *)(base + round256(vec * (size_t)k) + round256(vec));
+    double *d_beta = (double *)((char *)d_alpha + round256((size_t)nvec * k * sizeof(double)));
+    double2 *d_h = (double2 *)((char *)d_beta + round256((size_t)nvec * k * sizeof(double)));
+    cudaError_t e;
+    switch (dtype) {
+        case CHASE_F32:  e = run<float>(H, N, V0, nvec, k, dtype, workspace, d_alpha, d_beta, d_h, stream); break;
+        case CHASE_F64:  e = run<double>(H, N, V0, nvec, k, dtype, workspace, d_alpha, d_beta, d_h, stream); break;
+        case CHASE_C64:  e = run<float2>(H, N, V0, nvec, k, dtype, workspace, d_alpha, d_beta, d_h, stream); break;
+        default:         e = run<double2>(H, N, V0, nvec, k, dtype, workspace, d_alpha, d_beta, d_h, stream); break;
+    }
+    if (e != cudaSuccess) return e;
+    const size_t cb = (size_t)nvec * k * sizeof(double);
+    if ((e = cudaMemcpyAsync(alpha_host, d_alpha, cb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
+    if ((e = cudaMemcpyAsync(beta_host, d_beta, cb, cudaMemcpyDeviceToHost, stream)) != cudaSuccess) return e;
+    return cudaStreamSynchronize(stream);
+}
+
+bool lanczos_ritz(int k, const double *alpha, const double *beta, std::vector<double> &lam, std::vector<double> &w) {
+    std::vector<double> d(alpha, alpha + k), e(beta, beta + (k > 0 ? k - 1 : 0)), z;
+    if (!tridiag_ql_first_row(k, d, e, z)) return false;
+    lam = d;
+    w.resize(k);
+    for (int i = 0; i < k; ++i) w[i] = z[i] * z[i];
+    return true;
+}
+
+}  // namespace chase
