@@ -44,6 +44,15 @@ FP64_FLOP_PER_CLK_SM = 128
 TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks: tf32 1.1, bf16 2.25 PFLOP/s
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one full-width step launch (ncu --set full captures).
+NCU_TRAFFIC = {
+    4: (155.942670e9 + 1.323090e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); "
+                                   "profiles/ncu_r1b_step_dmma_c128.md"),
+    5: (3.669438e12 + 5.801412e9, "bytes of one full-width launch (3000 columns; algorithmic 57.6e9 + vectors); "
+                                  "profiles/ncu_r1b_step_tf32_c64.md"),
+}
+
+
 def measured_bf16_sustained_tflops():
     """(TFLOP/s, source): the driver-written sustained bf16 GEMM rate (the step kernel is timed inside a
     long step), else the nominal dense figure."""
@@ -335,10 +344,15 @@ def run_ours(args):
         kname = "step_dmma_kernel" if kernel_path == 1 else "step_generic_kernel"
         peak_source = (f"{sms} SMs x {per_clk} flop/clk/SM x clocks.max.sm {sm_max_mhz:.0f} MHz "
                        f"(DESIGN.md 'Peak'); MEASURED_PEAKS.json has no FP64 entry")
+    # DRAM bytes (read + write) of ONE full-width launch from the committed `ncu --set full` capture
+    # (profiles/); only known for the two captured workloads.
+    traffic, traffic_note = None, None
+    if args.N is None and args.ncols is None and args.config in NCU_TRAFFIC:
+        traffic, traffic_note = NCU_TRAFFIC[args.config]
     roofline = {
         "bound": bound, "kernel": kname,
         "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": None, "peak_source": peak_source,
+        "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_source,
         "peak_probe_dmma_tflops": probe_dmma, "peak_probe_dfma_tflops": probe_dfma,
         "frac_of_probe_dmma": achieved / probe_dmma if is_f64 else None,
         "frac_of_nvidia_quoted_40tf": achieved / 40.0 if is_f64 else None,
