@@ -35,7 +35,8 @@ class ChaseFilterError(RuntimeError):
 
 
 def lib_path() -> str:
-    return _build.LIB
+    """The in-tree library; CHASE_FILTER_LIB selects another build of the same sources."""
+    return os.environ.get("CHASE_FILTER_LIB") or _build.LIB
 
 
 def load() -> ctypes.CDLL:

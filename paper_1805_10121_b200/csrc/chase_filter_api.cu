@@ -52,7 +52,7 @@ size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtyp
     size_t bytes = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
     if (chase_filter_kernel_path(N, ncols, dtype) == 2) {
         // tcgen05 3xTF32 path: W, lo parts (complex: also -i V and its lo part) and H_lo (N x N)
-        bytes = (size_t)tf32_vector_blocks(dtype) * bytes + ((size_t)N * (size_t)N * w + 255) / 256 * 256;
+        bytes = (size_t)tf32_vector_blocks(dtype) * bytes + ((size_t)N * (size_t)N * w + 255) / 256 * 256 + 256;
     }
     return bytes;
 }

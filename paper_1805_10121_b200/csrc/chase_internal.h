@@ -55,6 +55,7 @@ struct Tf32Plan {
     chase_dtype_t dtype;
     int64_t N, ncols;
     void *buf[2], *lo[2], *rot[2], *rot_lo[2];  // [0]: the caller's V side, [1]: the workspace side
+    void *sync_ctr;                             // 4-byte counter of the producers' soft grid barrier
 };
 bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
 int tf32_vector_blocks(chase_dtype_t dtype);    // vector-sized blocks in the workspace besides H_lo

@@ -19,12 +19,6 @@ namespace {
 
 constexpr int kBlock = 256;
 
-template <typename T> struct Elem;
-template <> struct Elem<float>   { using real = float;  static constexpr bool cplx = false; };
-template <> struct Elem<double>  { using real = double; static constexpr bool cplx = false; };
-template <> struct Elem<float2>  { using real = float;  static constexpr bool cplx = true; };
-template <> struct Elem<double2> { using real = double; static constexpr bool cplx = true; };
-
 __device__ __forceinline__ double2 ld(const float *p, int64_t i)   { return make_double2((double)p[i], 0.0); }
 __device__ __forceinline__ double2 ld(const double *p, int64_t i)  { return make_double2(p[i], 0.0); }
 __device__ __forceinline__ double2 ld(const float2 *p, int64_t i)  { const float2 v = p[i]; return make_double2(v.x, v.y); }

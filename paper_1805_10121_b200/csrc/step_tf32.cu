@@ -30,6 +30,7 @@
 // by TMA: [row][16 floats of k] (64-byte rows, 8-row groups 512 B apart); one UMMA consumes 8 k.
 #include <cuda.h>
 
+#include <algorithm>
 #include <mutex>
 
 #include "chase_internal.h"
@@ -43,7 +44,10 @@ constexpr int KS = 16;            // floats of k per pipeline stage (two UMMA K 
 constexpr int TM = 128;           // (complex or real) rows per CTA tile = TMEM lanes
 constexpr int TN = 256;           // real B columns per CTA tile = TMEM columns
 constexpr int STAGES = 4;
-constexpr int CHUNK = 2;            // pipeline stages accumulated in TMEM before the sum moves to registers
+#ifndef TF32_CHUNK
+#define TF32_CHUNK 2
+#endif
+constexpr int CHUNK = TF32_CHUNK;            // pipeline stages accumulated in TMEM before the sum moves to registers
 constexpr int A_BYTES = TM * KS * 4;          // 8 KB
 constexpr int B_BYTES = TN * KS * 4;          // 16 KB
 constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi + lo of both: 48 KB
@@ -125,8 +129,14 @@ struct Tf32Params {
     float alpha, beta, c;
     const double *c_col;
     int use_beta;
+    unsigned *sync_ctr;                 // soft grid barrier counter (zeroed before the launch) or nullptr
 };
 
+#ifndef TF32_SYNC_STAGES
+#define TF32_SYNC_STAGES 64
+#endif
+constexpr int kSyncStages = TF32_SYNC_STAGES;   // producers meet every this many pipeline stages
+constexpr int kSyncMaxPolls = 512;              // bounded wait (~50 us): the barrier is only a hint
 constexpr int kGroupN = 8;
 __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
     const int per_group = kGroupN * tiles_m;
@@ -138,6 +148,25 @@ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int
     tn = first_n + r % gn;
 }
 
+// Soft grid barrier between the TMA producers of all CTAs (a performance hint, never needed for
+// correctness): arrive on a global counter and poll until `target` arrivals, for a bounded time.
+// Returns false if the wait timed out (the caller then stops syncing: some CTA is not running alongside).
+__device__ __forceinline__ bool soft_grid_sync(unsigned *ctr, unsigned target) {
+    atomicAdd(ctr, 1u);
+    for (int i = 0; i < kSyncMaxPolls; ++i) {
+        unsigned v;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+        if ((int)(v - target) >= 0) return true;
+        __nanosleep(64);
+    }
+    return false;
+}
+
+// Persistent: CTA b processes tiles b, b + gridDim.x, ... of the grouped raster (round r = the tiles
+// r * gridDim.x .. (r+1) * gridDim.x - 1, i.e. ~8 column tiles x ~18 row tiles that share H row panels and
+// X column panels in L2).  The resident CTAs only share those panels if they walk along k TOGETHER: the
+// L2 holds ~18 pipeline stages of the union stream, a tile lasts ~7500 stages.  So the producers meet at
+// a soft barrier at the start of every tile and every kSyncStages stages.
 template <bool CPLX>
 __global__ void __launch_bounds__(kThreads, 1)
 step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_constant__ CUtensorMap tmapA_lo,
@@ -154,11 +183,9 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
     const uint32_t tmem_slot = bar_base + 8 * (2 * STAGES + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int tile_m, tile_n;
-    tile_coords(blockIdx.x, p.tiles_m, p.tiles_n, tile_m, tile_n);
-    const int m0 = tile_m * TM, n0 = tile_n * COLS;
-    const int KT = (int)((p.KF + KS - 1) / KS);          // pipeline stages over k
-    const int NCH = (KT + CHUNK - 1) / CHUNK;            // TMEM accumulation chunks
+    const int total_tiles = p.tiles_m * p.tiles_n;
+    const int KT = (int)((p.KF + KS - 1) / KS);          // pipeline stages over k, per tile
+    const int NCH = (KT + CHUNK - 1) / CHUNK;            // TMEM accumulation chunks, per tile
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -184,57 +211,82 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
     if (warp == 0) {
         // ------------------------------------------------------------------ TMA producer
         if (lane == 0) {
-            for (int kt = 0; kt < KT; ++kt) {
-                const int s = kt % STAGES;
-                const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
-                if (kt >= STAGES) mbar_wait(empty, ((kt / STAGES) - 1) & 1);
-                const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
-                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
-                mbar_expect_tx(full, STAGE_BYTES);
-                const int k0 = kt * KS;
-                tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);          // 128 columns of H, 16 floats of k
-                tma_load_2d(sa_lo, &tmapA_lo, full, k0, m0);
-                tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
-                tma_load_2d(sb_lo, &tmapB_lo, full, k0, p.col0 + n0);
-                if (CPLX) {   // rows 128..255 of the B tile: -i X  (gives the imaginary part of A x)
-                    tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
-                    tma_load_2d(sb_lo + B_BYTES / 2, &tmapR_lo, full, k0, p.col0 + n0);
+            const int syncs_per_tile = (KT + kSyncStages - 1) / kSyncStages;
+            unsigned it = 0;                                  // stages filled so far (all tiles)
+            unsigned *sync_ctr = p.sync_ctr;
+            int round = 0;
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++round) {
+                int tile_m, tile_n;
+                tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+                const int m0 = tile_m * TM, n0 = tile_n * COLS;
+                const unsigned active = (unsigned)min((int)gridDim.x, total_tiles - round * (int)gridDim.x);
+                const unsigned sync_base = (unsigned)round * gridDim.x * (unsigned)syncs_per_tile;
+                for (int kt = 0; kt < KT; ++kt, ++it) {
+                    if (sync_ctr && kt % kSyncStages == 0 &&
+                        !soft_grid_sync(sync_ctr, sync_base + active * (unsigned)(kt / kSyncStages + 1)))
+                        sync_ctr = nullptr;
+                    const int s = it % STAGES;
+                    const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
+                    if (it >= STAGES) mbar_wait(empty, ((it / STAGES) - 1) & 1);
+                    const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
+                    const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
+                    const int k0 = kt * KS;
+#ifdef TF32_EXP_NOLO   // timing experiment only: the lo tiles are never loaded (results are wrong)
+                    mbar_expect_tx(full, STAGE_BYTES / 2);
+                    tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);
+                    tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
+                    if (CPLX) tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
+                    (void)sa_lo; (void)sb_lo;
+#else
+                    mbar_expect_tx(full, STAGE_BYTES);
+                    tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);          // 128 columns of H, 16 floats of k
+                    tma_load_2d(sa_lo, &tmapA_lo, full, k0, m0);
+                    tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
+                    tma_load_2d(sb_lo, &tmapB_lo, full, k0, p.col0 + n0);
+                    if (CPLX) {   // rows 128..255 of the B tile: -i X  (gives the imaginary part of A x)
+                        tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
+                        tma_load_2d(sb_lo + B_BYTES / 2, &tmapR_lo, full, k0, p.col0 + n0);
+                    }
+#endif
                 }
             }
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer
         if (lane == 0) {
-            int kt = 0;
-            for (int ch = 0; ch < NCH; ++ch) {
-                const int b = ch & 1;
-                if (ch >= 2) {   // the accumulator warps must have drained this buffer's previous chunk
-                    mbar_wait(bar_tempty + 8 * b, ((ch >> 1) - 1) & 1);
-                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                }
-                const uint32_t d = tmem_base + b * TN;
-                const int kt_end = min(KT, kt + CHUNK);
-                for (bool first = true; kt < kt_end; ++kt) {
-                    const int s = kt % STAGES;
-                    mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
-                    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
-                    const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
-#pragma unroll
-                    for (int ks = 0; ks < KS / 8; ++ks) {
-                        // K-major SWIZZLE_64B: 8-row groups 512 B apart; the 8-k slice ks starts 32 B into the row
-                        const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
-                        const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
-                        const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
-                        const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
-                        umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
-                        umma_tf32(d, al, bh, 1u);                 // lo * hi
-                        umma_tf32(d, ah, bh, 1u);                 // hi * hi
-                        first = false;
+            unsigned it = 0, gc = 0;                          // stages consumed / chunks issued so far (all tiles)
+            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+                int kt = 0;
+                for (int ch = 0; ch < NCH; ++ch, ++gc) {
+                    const int b = gc & 1;
+                    if (gc >= 2) {   // the accumulator warps must have drained this buffer's previous chunk
+                        mbar_wait(bar_tempty + 8 * b, ((gc >> 1) - 1) & 1);
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                     }
-                    umma_commit(bar_base + 8 * (STAGES + s));   // frees the smem stage when these MMAs retire
+                    const uint32_t d = tmem_base + b * TN;
+                    const int kt_end = min(KT, kt + CHUNK);
+                    for (bool first = true; kt < kt_end; ++kt, ++it) {
+                        const int s = it % STAGES;
+                        mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
+                        const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
+#pragma unroll
+                        for (int ks = 0; ks < KS / 8; ++ks) {
+                            // K-major SWIZZLE_64B: 8-row groups 512 B apart; the 8-k slice ks starts 32 B into the row
+                            const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
+                            const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
+                            const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
+                            const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
+                            umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
+                            umma_tf32(d, al, bh, 1u);                 // lo * hi
+                            umma_tf32(d, ah, bh, 1u);                 // hi * hi
+                            first = false;
+                        }
+                        umma_commit(bar_base + 8 * (STAGES + s));   // frees the smem stage when these MMAs retire
+                    }
+                    umma_commit(bar_tfull + 8 * b);                  // this chunk's accumulator is complete
                 }
-                umma_commit(bar_tfull + 8 * b);                  // this chunk's accumulator is complete
             }
         }
     } else {
@@ -245,44 +297,50 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
         const int quarter = warp & 3;                       // TMEM lanes this warp may access
         const int half = (warp - 2) >> 2;                   // which 128 of the 256 accumulator columns
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
-        float racc[TN / 2];
-#pragma unroll
-        for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
-        for (int ch = 0; ch < NCH; ++ch) {
-            const int b = ch & 1;
-            mbar_wait(bar_tfull + 8 * b, (ch >> 1) & 1);
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-            for (int j = 0; j < TN / 2 / 32; ++j) {
-                float t[32];
-                tmem_ld32(taddr + b * TN + j * 32, t);
-#pragma unroll
-                for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
-            }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_tempty + 8 * b);
-        }
-
-        const int64_t row = (int64_t)m0 + quarter * 32 + lane;
-        const bool row_ok = row < p.N;
         const float alpha = p.alpha, beta = p.beta;
+        unsigned gc = 0;                                     // chunks drained so far (all tiles)
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            int tile_m, tile_n;
+            tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+            const int m0 = tile_m * TM, n0 = tile_n * COLS;
+            float racc[TN / 2];
 #pragma unroll
-        for (int i = 0; i < TN / 2; ++i) {
-            // complex: half 0 owns the real parts, half 1 the imaginary parts of columns n0 .. n0+127
-            const int col = CPLX ? n0 + i : n0 + half * (TN / 2) + i;
-            if (col < p.n && row_ok) {
-                const float c = p.c_col ? (float)p.c_col[col] : p.c;
-                const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
-                float y = alpha * (racc[i] - c * p.X[off]);
-                if (p.use_beta) y = fmaf(beta, p.Y[off], y);
-                const float lo = y - tf32_hi(y);
-                p.Y[off] = y;
-                p.Y_lo[off] = lo;
-                if (CPLX) {   // -i y = (Im y, -Re y)
-                    const int64_t roff = off + (half ? -1 : 1);
-                    p.Yrot[roff] = half ? y : -y;
-                    p.Yrot_lo[roff] = half ? lo : -lo;
+            for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
+            for (int ch = 0; ch < NCH; ++ch, ++gc) {
+                const int b = gc & 1;
+                mbar_wait(bar_tfull + 8 * b, (gc >> 1) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (int j = 0; j < TN / 2 / 32; ++j) {
+                    float t[32];
+                    tmem_ld32(taddr + b * TN + j * 32, t);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_tempty + 8 * b);
+            }
+
+            const int64_t row = (int64_t)m0 + quarter * 32 + lane;
+            const bool row_ok = row < p.N;
+#pragma unroll
+            for (int i = 0; i < TN / 2; ++i) {
+                // complex: half 0 owns the real parts, half 1 the imaginary parts of columns n0 .. n0+127
+                const int col = CPLX ? n0 + i : n0 + half * (TN / 2) + i;
+                if (col < p.n && row_ok) {
+                    const float c = p.c_col ? (float)p.c_col[col] : p.c;
+                    const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
+                    float y = alpha * (racc[i] - c * p.X[off]);
+                    if (p.use_beta) y = fmaf(beta, p.Y[off], y);
+                    const float lo = y - tf32_hi(y);
+                    p.Y[off] = y;
+                    p.Y_lo[off] = lo;
+                    if (CPLX) {   // -i y = (Im y, -Re y)
+                        const int64_t roff = off + (half ? -1 : 1);
+                        p.Yrot[roff] = half ? y : -y;
+                        p.Yrot_lo[roff] = half ? lo : -lo;
+                    }
                 }
             }
         }
@@ -351,6 +409,18 @@ cudaError_t encode_kmajor(CUtensorMap *map, const void *base, int64_t KF, int64_
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+int sm_count() {
+    static int sms = 0;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+            sms = 148;
+    });
+    return sms;
+}
+
 template <bool CPLX>
 cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
                    cudaStream_t stream, const double *c_col) {
@@ -383,9 +453,16 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     p.c = (float)c;
     p.c_col = c_col;
     p.use_beta = use_beta;
+    p.sync_ctr = (unsigned *)plan->sync_ctr;
+    const int total_tiles = p.tiles_m * p.tiles_n;
+    const int grid = std::min(total_tiles, sm_count());      // persistent: one CTA per SM
+    if (p.sync_ctr) {
+        cudaError_t e = cudaMemsetAsync(p.sync_ctr, 0, sizeof(unsigned), stream);
+        if (e != cudaSuccess) return e;
+    }
     const CUtensorMap *B = (const CUtensorMap *)plan->tmap_B[0];   // [hi V, hi W, lo V, lo W, rot V, rot W, rot_lo V, rot_lo W]
     const int r_hi = CPLX ? 4 + src : src, r_lo = CPLX ? 6 + src : 2 + src;
-    step_tf32_kernel<CPLX><<<(unsigned)(p.tiles_m * p.tiles_n), kThreads, SMEM_TOTAL, stream>>>(
+    step_tf32_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM_TOTAL, stream>>>(
         *(const CUtensorMap *)plan->tmap_A[0], *(const CUtensorMap *)plan->tmap_A[1], B[src], B[2 + src], B[r_hi],
         B[r_lo], p);
     count_launch();
@@ -422,6 +499,8 @@ cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H,
         plan->rot[0] = plan->rot[1] = plan->rot_lo[0] = plan->rot_lo[1] = nullptr;
     }
     void *H_lo = base + (size_t)tf32_vector_blocks(dtype) * vb;
+    const size_t hb = ((size_t)N * (size_t)KF * 4 + 255) / 256 * 256;
+    plan->sync_ctr = (char *)H_lo + hb;          // 256 bytes after H_lo: the soft grid barrier counter
 
     // lo part of H (x - tf32(x)) and, for V_0, lo (and -i V_0 with its lo part)
     split_lo_kernel<<<148 * 8, 256, 0, stream>>>((const float *)H, (float *)H_lo, N * KF);
