@@ -46,9 +46,9 @@ extern "C" {
 #endif
 
 typedef enum {
-    CHASE_F32 = 0,  /* float,                 FP32 FMA arithmetic */
+    CHASE_F32 = 0,  /* float,                 tcgen05 3xTF32 tensor path when N % 4 == 0, else FP32 FMA */
     CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N % 16 == 0) */
-    CHASE_C64 = 2,  /* interleaved float2,    FP32 FMA arithmetic */
+    CHASE_C64 = 2,  /* interleaved float2,    tcgen05 3xTF32 tensor path when N % 2 == 0, else FP32 FMA */
     CHASE_C128 = 3  /* interleaved double2,   FP64 (DMMA tensor path when N % 8 == 0) */
 } chase_dtype_t;
 
@@ -63,8 +63,8 @@ enum {
 };
 
 /* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype` (the W of
- * Alg. 4), rounded up to 256 bytes; on the tcgen05 3xTF32 path (see chase_filter_kernel_path)
- * three such buffers plus one N x N buffer (low-order parts of the iterates and of H).
+ * Alg. 4), rounded up to 256 bytes (plus 256 bytes on the tcgen05 3xTF32 path, see
+ * chase_filter_kernel_path: the counter of a soft barrier between the persistent CTAs).
  * 0 if an argument is invalid. */
 size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
@@ -76,8 +76,8 @@ size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtyp
  *   workspace  DEVICE, >= chase_filter_workspace_bytes(...) bytes, 16-byte aligned; contents
  *              undefined on entry and exit
  *   stream     cudaStream_t
- * Enqueues exactly max(degrees) step kernels (plus one small copy kernel if any degree is
- * odd) and returns without synchronising. */
+ * Enqueues exactly max(degrees) step kernels (plus one device copy per run of odd-degree
+ * columns; on the 3xTF32 path a 4-byte memset before each kernel) and returns without synchronising. */
 int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                     double a, double b, double lambda1, chase_dtype_t dtype,
                     void *workspace, size_t workspace_bytes, void *stream);
@@ -170,7 +170,7 @@ int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, cons
 
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
  * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
- * N % 4 == 0; needs the larger workspace chase_filter_workspace_bytes reports), 0 = generic FMA
+ * N % 4 == 0; FP32 operands split on chip into two TF32 parts, FP32 accumulation), 0 = generic FMA
  * kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1 turns 2
  * into 0.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);

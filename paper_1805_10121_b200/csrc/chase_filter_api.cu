@@ -50,10 +50,7 @@ size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtyp
     size_t w = elem_bytes(dtype);
     if (w == 0 || N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return 0;
     size_t bytes = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
-    if (chase_filter_kernel_path(N, ncols, dtype) == 2) {
-        // tcgen05 3xTF32 path: W, lo parts (complex: also -i V and its lo part) and H_lo (N x N)
-        bytes = (size_t)tf32_vector_blocks(dtype) * bytes + ((size_t)N * (size_t)N * w + 255) / 256 * 256 + 256;
-    }
+    if (chase_filter_kernel_path(N, ncols, dtype) == 2) bytes += 256;   // tcgen05 path: soft grid barrier counter
     return bytes;
 }
 
@@ -140,11 +137,20 @@ namespace chase {
 int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha,
                            double beta, double c, const double *c_col, int use_beta, chase_dtype_t dtype,
                            cudaStream_t stream) {
-    if (chase_filter_kernel_path(N, ncols, dtype) == 1) {
+    const int path = chase_filter_kernel_path(N, ncols, dtype);
+    if (path == 1) {
         DmmaPlan plan;
         cudaError_t e = dmma_plan_create(&plan, dtype, H, N, const_cast<void *>(X), Y, ncols);
         if (e != cudaSuccess) return (int)e;
         e = dmma_launch_step(&plan, 0, 0, alpha, beta, c, use_beta, stream, c_col);
+        return (int)e;
+    }
+    if (path == 2 && ncols >= 32) {   // a 128 x 128 (256) tensor tile only pays with enough columns
+        Tf32Plan plan;
+        cudaError_t e = tf32_plan_create(&plan, dtype, H, N, const_cast<void *>(X), Y, 0, ncols, stream);
+        if (e != cudaSuccess) return (int)e;
+        plan.sync_ctr = tf32_shared_sync_counter();     // may be null: the barrier is only a hint
+        e = tf32_launch_step(&plan, 0, 0, alpha, beta, c, use_beta, stream, c_col);
         return (int)e;
     }
     StepArgs sa;

@@ -50,19 +50,22 @@ cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double al
 
 // tcgen05 3xTF32 kernels (CHASE_C64 with N % 2 == 0, CHASE_F32 with N % 4 == 0).
 struct Tf32Plan {
-    alignas(64) unsigned char tmap_A[2][128];   // H, H_lo
-    alignas(64) unsigned char tmap_B[8][128];   // hi V/W, lo V/W, rot V/W, rot_lo V/W
+    alignas(64) unsigned char tmap_A[128];      // H viewed K-major (Hermitian: row m along k = conj of column m)
+    alignas(64) unsigned char tmap_B[2][128];   // [0]: the caller's V, [1]: the workspace W
     chase_dtype_t dtype;
     int64_t N, ncols;
-    void *buf[2], *lo[2], *rot[2], *rot_lo[2];  // [0]: the caller's V side, [1]: the workspace side
+    void *buf[2];
     void *sync_ctr;                             // 4-byte counter of the producers' soft grid barrier
 };
 bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
 int tf32_vector_blocks(chase_dtype_t dtype);    // vector-sized blocks in the workspace besides H_lo
-// Carves the workspace, launches the two pre-pass kernels (lo parts of H and V_0, -i V_0) and
-// encodes the tensor maps.  vb = bytes of one N x ncols block rounded up to 256.
+// Encodes the tensor maps.  vb = bytes of one N x ncols block rounded up to 256; the 256 bytes after
+// it hold the soft-barrier counter.
 cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V,
                              void *workspace, size_t vb, int64_t ncols, cudaStream_t stream);
+// A process-wide 256-byte device buffer for the soft barrier of launches that have no workspace
+// (chase_hemm, chase_residuals, chase_lanczos); nullptr if it cannot be allocated.
+void *tf32_shared_sync_counter();
 cudaError_t tf32_launch_step(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c,
                              int use_beta, cudaStream_t stream, const double *c_col = nullptr);
 

@@ -7,9 +7,12 @@
 // (what kind::tf32 reads from an fp32 word), lo = x - hi (exact in fp32).  The product is
 // evaluated as hi*lo + lo*hi + hi*hi (lo*lo ~ 2^-22 relative is dropped): three tcgen05.mma per
 // k-slice into ONE fp32 accumulator in tensor memory, which restores fp32-level accuracy (plain
-// single-pass TF32, 2^-11 per operand, would not meet the 1e-4 bound).  The lo parts live in
-// global memory: H_lo is computed once per chase_filter call, the lo part of each new iterate is
-// written by the epilogue that produces it.
+// single-pass TF32, 2^-11 per operand, would not meet the 1e-4 bound).
+//
+// Only the fp32 data itself crosses L2: TMA brings the raw H and X tiles (they serve as the hi
+// operands, the tensor core ignores the low mantissa bits) and two converter warps derive the lo
+// tiles -- and for complex64 the rotated tile -i X -- in shared memory.  The split is element-wise
+// and the rotation stays inside a 16-byte chunk, so both are oblivious of the 64-byte swizzle.
 //
 // Both operands are K-major.  For A this uses that H is Hermitian (reading G9): row m of
 // H along k is the conjugate of column m, which is contiguous in the column-major storage.
@@ -17,15 +20,14 @@
 //   complex64: a REAL GEMM over the interleaved index kk = 2k + {0, 1}:
 //     A2[m][kk]  = column m of H as floats    = (Re A[m,k], -Im A[m,k])      (conjugate of H[k,m])
 //     B1[kk][j]  = column j of X as floats    = (Re x, Im x)
-//     B2[kk][j]  = column j of Xrot = -i X    = (Im x, -Re x)
+//     B2[kk][j]  = column j of -i X           = (Im x, -Re x)
 //     A2 . B1 = Re(A x),  A2 . B2 = Im(A x):  D = 128 complex rows x [128 Re | 128 Im] columns.
-//   Xrot (and the lo parts) of every iterate are written by the epilogue that produces it.
 //
-// Warp roles (320 threads, 1 CTA / SM): warp 0 = TMA producer (one lane), warp 1 = TMEM
-// allocator + MMA issuer (one lane), warps 2-9 = accumulator/epilogue warps (TMEM lane quarter =
-// warp % 4, column half = (warp-2)/4).  The MMA issuer accumulates CHUNK stages into one of two
-// TMEM buffers; the accumulator warps add each finished chunk into fp32 registers (round to
-// nearest) while the tensor core fills the other buffer, then run the fused epilogue.
+// Warp roles (384 threads, 1 persistent CTA / SM): warp 0 = TMA producer (one lane), warp 1 = TMEM
+// allocator + MMA issuer (one lane), warps 2-3 = converters, warps 4-11 = accumulator/epilogue warps
+// (TMEM lane quarter = warp % 4, column half = (warp-4)/4).  The MMA issuer accumulates CHUNK stages
+// into one of two TMEM buffers; the accumulator warps add each finished chunk into fp32 registers
+// (round to nearest) while the tensor core fills the other buffer, then run the fused epilogue.
 // Shared-memory operand tiles are the canonical K-major SWIZZLE_64B UMMA layout written directly
 // by TMA: [row][16 floats of k] (64-byte rows, 8-row groups 512 B apart); one UMMA consumes 8 k.
 #include <cuda.h>
@@ -38,14 +40,16 @@
 namespace chase {
 namespace {
 
+constexpr int kConvWarps = 2;      // converter warps (lo parts and -i X, in shared memory)
+constexpr int kFirstAccWarp = 4;   // multiple of 4: TMEM lane quarter = warp % 4
 constexpr int kAccWarps = 8;       // accumulator / epilogue warps: 4 TMEM lane quarters x 2 column halves
-constexpr int kThreads = (2 + kAccWarps) * 32;
+constexpr int kThreads = (kFirstAccWarp + kAccWarps) * 32;
 constexpr int KS = 16;            // floats of k per pipeline stage (two UMMA K = 8 slices)
 constexpr int TM = 128;           // (complex or real) rows per CTA tile = TMEM lanes
 constexpr int TN = 256;           // real B columns per CTA tile = TMEM columns
 constexpr int STAGES = 4;
 #ifndef TF32_CHUNK
-#define TF32_CHUNK 2
+#define TF32_CHUNK 4
 #endif
 constexpr int CHUNK = TF32_CHUNK;            // pipeline stages accumulated in TMEM before the sum moves to registers
 constexpr int A_BYTES = TM * KS * 4;          // 8 KB
@@ -116,11 +120,23 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
+    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float4 split_lo(float4 v) {
+    return make_float4(v.x - tf32_hi(v.x), v.y - tf32_hi(v.y), v.z - tf32_hi(v.z), v.w - tf32_hi(v.w));
+}
+__device__ __forceinline__ float4 rot_mi(float4 v) { return make_float4(v.y, -v.x, v.w, -v.z); }   // -i (x + iy) pairs
 
 
 struct Tf32Params {
     const float *X;                     // source iterate, first active column
-    float *Y, *Y_lo, *Yrot, *Yrot_lo;   // destination iterate, its lo part, -i*iterate and its lo part (rot: complex only)
+    float *Y;                           // destination iterate (holds V_{k-1}, becomes V_{k+1}), first active column
     int64_t N;                          // matrix order
     int64_t KF;                         // floats along k per column: 2N (complex) or N (real)
     int n;                              // active columns
@@ -169,18 +185,17 @@ __device__ __forceinline__ bool soft_grid_sync(unsigned *ctr, unsigned target) {
 // a soft barrier at the start of every tile and every kSyncStages stages.
 template <bool CPLX>
 __global__ void __launch_bounds__(kThreads, 1)
-step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_constant__ CUtensorMap tmapA_lo,
-                 const __grid_constant__ CUtensorMap tmapB_hi, const __grid_constant__ CUtensorMap tmapB_lo,
-                 const __grid_constant__ CUtensorMap tmapR_hi, const __grid_constant__ CUtensorMap tmapR_lo,
+step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
                  const Tf32Params p) {
     constexpr int COLS = CPLX ? TN / 2 : TN;      // (complex or real) columns per tile
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[S], empty[S], tfull[2], tempty[2], tmem slot
-    const uint32_t bar_tfull = bar_base + 8 * (2 * STAGES);
-    const uint32_t bar_tempty = bar_base + 8 * (2 * STAGES + 2);
-    const uint32_t tmem_slot = bar_base + 8 * (2 * STAGES + 4);
+    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[S], empty[S], conv[S], tfull[2], tempty[2], tmem slot
+    const uint32_t bar_conv = bar_base + 8 * (2 * STAGES);
+    const uint32_t bar_tfull = bar_base + 8 * (3 * STAGES);
+    const uint32_t bar_tempty = bar_base + 8 * (3 * STAGES + 2);
+    const uint32_t tmem_slot = bar_base + 8 * (3 * STAGES + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int total_tiles = p.tiles_m * p.tiles_n;
@@ -191,6 +206,7 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
         for (int s = 0; s < STAGES; ++s) {
             mbar_init(bar_base + 8 * s, 1);              // full: producer's expect_tx arrive
             mbar_init(bar_base + 8 * (STAGES + s), 1);   // empty: one tcgen05.commit arrive
+            mbar_init(bar_conv + 8 * s, kConvWarps);     // conv: lo / rot tiles written by every converter warp
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_tfull + 8 * b, 1);             // chunk accumulator complete (tcgen05.commit)
@@ -231,23 +247,11 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
                     const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
                     const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
                     const int k0 = kt * KS;
-#ifdef TF32_EXP_NOLO   // timing experiment only: the lo tiles are never loaded (results are wrong)
-                    mbar_expect_tx(full, STAGE_BYTES / 2);
-                    tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);
-                    tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
-                    if (CPLX) tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
+                    // raw fp32 tiles only: 128 columns of H and 128 (complex) / 256 (real) columns of X, 16 floats of k
+                    mbar_expect_tx(full, A_BYTES + (CPLX ? B_BYTES / 2 : B_BYTES));
+                    tma_load_2d(sa_hi, &tmapA, full, k0, m0);
+                    tma_load_2d(sb_hi, &tmapB, full, k0, p.col0 + n0);
                     (void)sa_lo; (void)sb_lo;
-#else
-                    mbar_expect_tx(full, STAGE_BYTES);
-                    tma_load_2d(sa_hi, &tmapA_hi, full, k0, m0);          // 128 columns of H, 16 floats of k
-                    tma_load_2d(sa_lo, &tmapA_lo, full, k0, m0);
-                    tma_load_2d(sb_hi, &tmapB_hi, full, k0, p.col0 + n0);
-                    tma_load_2d(sb_lo, &tmapB_lo, full, k0, p.col0 + n0);
-                    if (CPLX) {   // rows 128..255 of the B tile: -i X  (gives the imaginary part of A x)
-                        tma_load_2d(sb_hi + B_BYTES / 2, &tmapR_hi, full, k0, p.col0 + n0);
-                        tma_load_2d(sb_lo + B_BYTES / 2, &tmapR_lo, full, k0, p.col0 + n0);
-                    }
-#endif
                 }
             }
         }
@@ -267,7 +271,8 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
                     const int kt_end = min(KT, kt + CHUNK);
                     for (bool first = true; kt < kt_end; ++kt, ++it) {
                         const int s = it % STAGES;
-                        mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);
+                        mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);      // TMA tiles landed
+                        mbar_wait(bar_conv + 8 * s, (it / STAGES) & 1);      // lo / rot tiles written
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                         const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
                         const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
@@ -289,13 +294,55 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
                 }
             }
         }
-    } else {
+    } else if (warp < 2 + kConvWarps) {
+        // ------------------------------------------------------------------ converter warps
+        // Stage layout: [A raw | A lo | B hi (complex: X raw, -iX) | B lo (complex: X lo, (-iX) lo)].
+        constexpr int CT = kConvWarps * 32;
+        const int ct = threadIdx.x - 64;
+        unsigned it = 0;
+        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+            for (int kt = 0; kt < KT; ++kt, ++it) {
+                const int s = it % STAGES;
+                mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);
+                const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
+                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
+                {
+#pragma unroll
+                for (int i = 0; i < A_BYTES / 16 / CT; ++i) {
+                    const uint32_t off = (uint32_t)(ct + i * CT) * 16;
+                    sts128(sa_lo + off, split_lo(lds128(sa_hi + off)));
+                }
+                if (CPLX) {
+#pragma unroll
+                    for (int i = 0; i < B_BYTES / 2 / 16 / CT; ++i) {
+                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
+                        const float4 v = lds128(sb_hi + off);
+                        const float4 lo = split_lo(v);
+                        sts128(sb_lo + off, lo);
+                        sts128(sb_hi + B_BYTES / 2 + off, rot_mi(v));
+                        sts128(sb_lo + B_BYTES / 2 + off, rot_mi(lo));
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < B_BYTES / 16 / CT; ++i) {
+                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
+                        sts128(sb_lo + off, split_lo(lds128(sb_hi + off)));
+                    }
+                }
+                }
+                // generic-proxy writes -> visible to the tensor core's async-proxy reads
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_conv + 8 * s);
+            }
+        }
+    } else if (warp >= kFirstAccWarp) {
         // ------------------------------------------------------------------ accumulator / epilogue warps
         // The tensor core's fp32 accumulation rounds toward zero, a bias that grows with the length
         // of the accumulation chain; so the chain is cut into chunks of CHUNK stages, and the chunk
         // sums are added here in registers with round-to-nearest.
         const int quarter = warp & 3;                       // TMEM lanes this warp may access
-        const int half = (warp - 2) >> 2;                   // which 128 of the 256 accumulator columns
+        const int half = (warp - kFirstAccWarp) >> 2;       // which 128 of the 256 accumulator columns
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
         const float alpha = p.alpha, beta = p.beta;
         unsigned gc = 0;                                     // chunks drained so far (all tiles)
@@ -333,14 +380,7 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
                     const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
                     float y = alpha * (racc[i] - c * p.X[off]);
                     if (p.use_beta) y = fmaf(beta, p.Y[off], y);
-                    const float lo = y - tf32_hi(y);
                     p.Y[off] = y;
-                    p.Y_lo[off] = lo;
-                    if (CPLX) {   // -i y = (Im y, -Re y)
-                        const int64_t roff = off + (half ? -1 : 1);
-                        p.Yrot[roff] = half ? y : -y;
-                        p.Yrot_lo[roff] = half ? lo : -lo;
-                    }
                 }
             }
         }
@@ -350,28 +390,6 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA_hi, const __grid_cons
     __syncthreads();
     if (warp == 1) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(2 * TN) : "memory");
-    }
-}
-
-// Pre-passes, once per call.  lo[i] = x[i] - hi(x[i]) (H, and a real V0) ...
-__global__ void __launch_bounds__(256) split_lo_kernel(const float *__restrict__ x, float *__restrict__ lo, int64_t count) {
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) {
-        const float v = x[i];
-        lo[i] = v - tf32_hi(v);
-    }
-}
-// ... and for a complex V0 also rot = -i x and its lo part.
-__global__ void __launch_bounds__(256) split_rot_kernel(const float2 *__restrict__ x, float2 *__restrict__ lo,
-                                                         float2 *__restrict__ rot, float2 *__restrict__ rot_lo,
-                                                         int64_t count) {
-    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < count; i += stride) {
-        const float2 v = x[i];
-        const float lr = v.x - tf32_hi(v.x), li = v.y - tf32_hi(v.y);
-        lo[i] = make_float2(lr, li);
-        rot[i] = make_float2(v.y, -v.x);
-        rot_lo[i] = make_float2(li, -lr);
     }
 }
 
@@ -439,9 +457,6 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     Tf32Params p;
     p.X = (const float *)plan->buf[src] + (size_t)s * col_floats;
     p.Y = (float *)plan->buf[dst] + (size_t)s * col_floats;
-    p.Y_lo = (float *)plan->lo[dst] + (size_t)s * col_floats;
-    p.Yrot = CPLX ? (float *)plan->rot[dst] + (size_t)s * col_floats : nullptr;
-    p.Yrot_lo = CPLX ? (float *)plan->rot_lo[dst] + (size_t)s * col_floats : nullptr;
     p.N = plan->N;
     p.KF = plan->N * FL;
     p.n = (int)n;
@@ -460,11 +475,8 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
         cudaError_t e = cudaMemsetAsync(p.sync_ctr, 0, sizeof(unsigned), stream);
         if (e != cudaSuccess) return e;
     }
-    const CUtensorMap *B = (const CUtensorMap *)plan->tmap_B[0];   // [hi V, hi W, lo V, lo W, rot V, rot W, rot_lo V, rot_lo W]
-    const int r_hi = CPLX ? 4 + src : src, r_lo = CPLX ? 6 + src : 2 + src;
     step_tf32_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM_TOTAL, stream>>>(
-        *(const CUtensorMap *)plan->tmap_A[0], *(const CUtensorMap *)plan->tmap_A[1], B[src], B[2 + src], B[r_hi],
-        B[r_lo], p);
+        *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
     count_launch();
     return cudaGetLastError();
 }
@@ -478,50 +490,38 @@ bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     return false;
 }
 
-// Workspace layout: [W | V_lo | W_lo | (complex: Vrot | Wrot | Vrot_lo | Wrot_lo) | H_lo], vector blocks of vb bytes.
-int tf32_vector_blocks(chase_dtype_t dtype) { return dtype == CHASE_C64 ? 7 : 3; }
+// Workspace layout: [W (one N x ncols block, vb bytes) | 256 bytes holding the soft-barrier counter].
+int tf32_vector_blocks(chase_dtype_t) { return 1; }
 
 cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V,
-                             void *workspace, size_t vb, int64_t ncols, cudaStream_t stream) {
+                             void *workspace, size_t vb, int64_t ncols, cudaStream_t) {
     const bool cplx = dtype == CHASE_C64;
-    const int FL = cplx ? 2 : 1;
-    const int64_t KF = N * FL;
-    char *base = (char *)workspace;
+    const int64_t KF = N * (cplx ? 2 : 1);
     plan->dtype = dtype;
     plan->N = N;
     plan->ncols = ncols;
-    plan->buf[0] = V;            plan->buf[1] = base;
-    plan->lo[0] = base + vb;     plan->lo[1] = base + 2 * vb;
-    if (cplx) {
-        plan->rot[0] = base + 3 * vb;     plan->rot[1] = base + 4 * vb;
-        plan->rot_lo[0] = base + 5 * vb;  plan->rot_lo[1] = base + 6 * vb;
-    } else {
-        plan->rot[0] = plan->rot[1] = plan->rot_lo[0] = plan->rot_lo[1] = nullptr;
-    }
-    void *H_lo = base + (size_t)tf32_vector_blocks(dtype) * vb;
-    const size_t hb = ((size_t)N * (size_t)KF * 4 + 255) / 256 * 256;
-    plan->sync_ctr = (char *)H_lo + hb;          // 256 bytes after H_lo: the soft grid barrier counter
-
-    // lo part of H (x - tf32(x)) and, for V_0, lo (and -i V_0 with its lo part)
-    split_lo_kernel<<<148 * 8, 256, 0, stream>>>((const float *)H, (float *)H_lo, N * KF);
-    count_launch();
-    if (cplx)
-        split_rot_kernel<<<148 * 8, 256, 0, stream>>>((const float2 *)V, (float2 *)plan->lo[0], (float2 *)plan->rot[0],
-                                                       (float2 *)plan->rot_lo[0], N * ncols);
-    else
-        split_lo_kernel<<<148 * 8, 256, 0, stream>>>((const float *)V, (float *)plan->lo[0], N * ncols);
-    count_launch();
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
-
-    if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A[0], H, KF, N, TM)) != cudaSuccess) return e;
-    if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A[1], H_lo, KF, N, TM)) != cudaSuccess) return e;
-    void *bufs[8] = {plan->buf[0], plan->buf[1], plan->lo[0], plan->lo[1],
-                     plan->rot[0], plan->rot[1], plan->rot_lo[0], plan->rot_lo[1]};
-    for (int i = 0; i < (cplx ? 8 : 4); ++i)
-        if ((e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], bufs[i], KF, ncols, cplx ? TN / 2 : TN)) != cudaSuccess)
+    plan->buf[0] = V;
+    plan->buf[1] = workspace;
+    plan->sync_ctr = (workspace && vb) ? (char *)workspace + vb : nullptr;
+    cudaError_t e;
+    if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A, H, KF, N, TM)) != cudaSuccess) return e;
+    for (int i = 0; i < 2; ++i)
+        if (plan->buf[i] &&
+            (e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], plan->buf[i], KF, ncols, cplx ? TN / 2 : TN)) != cudaSuccess)
             return e;
     return cudaSuccess;
+}
+
+void *tf32_shared_sync_counter() {
+    static void *buf = nullptr;
+    static std::once_flag once;
+    std::call_once(once, [] {
+        if (cudaMalloc(&buf, 256) != cudaSuccess) {
+            buf = nullptr;
+            (void)cudaGetLastError();
+        }
+    });
+    return buf;
 }
 
 cudaError_t tf32_launch_step(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c,

@@ -88,6 +88,34 @@ def test_generic_shapes_all_dtypes(dtype, N, ncols):
     assert_parity(run_gpu(w), run_oracle(w), dtype)
 
 
+@pytest.mark.parametrize("dtype,N,ncols", [
+    (torch.complex64, 770, 300),     # N % 2 == 0 only: ragged row tile, 3 column tiles
+    (torch.float32, 1036, 530),      # N % 4 == 0 only: 3 column tiles of 256
+    (torch.complex64, 2560, 1000),   # 20 x 8 = 160 tiles > 148 SMs: second round of the persistent loop
+])
+def test_tf32_path_shapes(dtype, N, ncols):
+    """tcgen05 3xTF32 kernel (kernel path 2): ragged tiles, several rounds, mixed degrees incl. 0 and odd."""
+    w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
+    assert pkg.chase_filter_kernel_path(N, ncols, dtype) == 2
+    rng = np.random.default_rng(5)
+    deg = torch.tensor(np.sort(rng.integers(0, 9, size=ncols)).astype(np.int32))
+    got = run_gpu(w, degrees=deg)
+    assert_parity(got, run_oracle(w, degrees=deg.numpy()), dtype)
+
+
+def test_tf32_launch_count_and_workspace():
+    """One step kernel per degree on the tensor path too; scratch = one vector block + 256 bytes."""
+    N, n = 512, 64
+    w = W.make_config(5, N=N, ncols=n)
+    assert pkg.chase_filter_workspace_bytes(N, n, w.dtype) == N * n * 8 + 256
+    H, V = to_device(w.H), to_device(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(N, n, w.dtype), dtype=torch.uint8, device=_dev())
+    before = pkg.chase_filter_launch_count()
+    pkg.chase_filter_ws(H, V, w.degrees, w.a, w.b, w.lambda1, ws)
+    torch.cuda.synchronize()
+    assert pkg.chase_filter_launch_count() - before == int(w.degrees.max())
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.complex128])
 def test_odd_zero_and_one_degrees(dtype):
     """Readings G5/G6: degree 0 untouched, degree 1 = first step only, odd degrees copied back."""

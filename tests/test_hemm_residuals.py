@@ -50,7 +50,8 @@ def _dev(x):
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("dtype,N,n", [(torch.complex128, 520, 77), (torch.float64, 1040, 150),
-                                        (torch.complex64, 300, 33), (torch.float32, 203, 20),
+                                        (torch.complex64, 300, 33), (torch.float32, 203, 20), (torch.float32, 516, 70),
+                                        (torch.complex64, 1282, 140),
                                         (torch.complex128, 203, 20)])
 def test_gpu_hemm_and_residuals(dtype, N, n):
     tol = 1e-12 if dtype in (torch.complex128, torch.float64) else 1e-4
