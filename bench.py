@@ -48,8 +48,8 @@ TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks
 NCU_TRAFFIC = {
     4: (155.942670e9 + 1.323090e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); "
                                    "profiles/ncu_r1b_step_dmma_c128.md"),
-    5: (3.669438e12 + 5.801412e9, "bytes of one full-width launch (3000 columns; algorithmic 57.6e9 + vectors); "
-                                  "profiles/ncu_r1b_step_tf32_c64.md"),
+    5: (129.506315e9 + 1.473567e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
+                                   "profiles/ncu_r1c_step_tf32_c64.md"),
 }
 
 
@@ -75,6 +75,7 @@ def parse_args():
     ap.add_argument("--ncols", type=int, default=None)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-aux", action="store_true", help="skip the hemm / residuals / Lanczos timings")
     ap.add_argument("--sample-cols", type=int, default=16)
     ap.add_argument("--sample-degree", type=int, default=8)
     return ap.parse_args()
@@ -220,6 +221,42 @@ def oracle_sample_run(Hn: np.ndarray, Vn: np.ndarray, degree: int, w):
     out = oracle.chase_filter(Hn, Vn, deg, w.a, w.b, w.lambda1)
     dt = time.perf_counter() - t0
     return dt, f * float(Hn.shape[0]) ** 2 * Vn.shape[1] * degree, out
+
+
+def time_aux_ops(pkg, w, Y, device):
+    """Device times of chase_hemm (Rayleigh-Ritz A Q^, all columns), chase_residuals and chase_lanczos
+    (k = 25, 1 + 4 runs; Table 1 defaults) on the bench workload.  One warm-up, one timed call each."""
+    N, n, dtype = w.N, w.ncols, w.dtype
+    f = 8.0 if dtype.is_complex else 2.0
+
+    def timed(fn):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    out = {}
+    ms = timed(lambda: pkg.chase_hemm(w.H, w.V0, Y))
+    out["chase_hemm"] = {"ms": ms, "gflops": f * N * N * n / ms * 1e-6, "ncols": n}
+    ritz = np.linspace(w.lambda1, w.a, n)
+    rws = torch.empty(pkg.chase_residuals_workspace_bytes(N, n, dtype), dtype=torch.uint8, device=device)
+    ms = timed(lambda: pkg.chase_residuals(w.H, w.V0, ritz, workspace=rws))
+    out["chase_residuals"] = {"ms": ms, "gflops": f * N * N * n / ms * 1e-6, "ncols": n}
+    del rws
+    k, nruns = 25, 5
+    lws = torch.empty(pkg.chase_lanczos_workspace_bytes(N, nruns, k, dtype), dtype=torch.uint8, device=device)
+    V0 = W.as_colmajor(w.V0[:, :nruns])
+    res = {}
+    ms = timed(lambda: res.update(ab=pkg.chase_lanczos(w.H, V0, k, workspace=lws)))
+    b_sup, mu1, mune = pkg.chase_spectral_estimates(res["ab"][0], res["ab"][1], N, n)
+    h_bytes = N * N * w.H.element_size()
+    out["chase_lanczos"] = {"ms": ms, "k": k, "runs": nruns, "hbm_gbs_over_H": k * h_bytes / ms * 1e-6,
+                            "b_sup": b_sup, "mu_1": mu1, "mu_nev_nex": mune}
+    return out
 
 
 # ----------------------------------------------------------------------------------------------
@@ -378,6 +415,11 @@ def run_ours(args):
                         "sample": sample, "seconds": dt}
         parity = {"rel_fro_vs_oracle": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)), "sample": sample}
 
+    # ---- aux: the other entry points on the same workload, device-timed --------------
+    aux = None
+    if rank == 0 and world == 1 and not args.no_aux:
+        aux = time_aux_ops(pkg, w, V, device)
+
     # ---- e2e: HOST buffers through chase_filter_host (H2D + filter + D2H inside the timed call) --
     e2e = None
     if not args.no_e2e:
@@ -407,7 +449,7 @@ def run_ours(args):
                                                                torch.float32: "f32"}[dtype],
             "data": "synthetic", "config": workload_config(args, w, world), "clocks": clocks,
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
-            "parity": parity, "wall_s_timed_region": t_wall,
+            "parity": parity, "aux_ops": aux, "wall_s_timed_region": t_wall,
             "fraction_of_fp64_peak": roofline["frac"] if is_f64 else None,
         }
         print(json.dumps(line))
