@@ -45,6 +45,8 @@
 extern "C" {
 #endif
 
+#define CHASE_MAX_RANKS 16   /* most GPUs one row-sharded filter spans (chase_filter_rows_*) */
+
 typedef enum {
     CHASE_F32 = 0,  /* float,                 tcgen05 3xTF32 tensor path when N % 4 == 0, else FP32 FMA */
     CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N % 16 == 0) */
@@ -167,6 +169,53 @@ int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nruns, int32
                   double *alpha, double *beta, void *workspace, size_t workspace_bytes, void *stream);
 int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, const double *beta, int64_t N,
                              double nev_nex, double sigma, double *b_sup, double *mu_1, double *mu_ne);
+
+/* Row-sharded path for matrices that exceed one GPU (SURVEY 8(e) option 2; the paper's block
+ * distribution of A, Fig. 3): one process per GPU, rank r owns the row block
+ * [row0, row0 + nrows) of H as an nrows x N column-major matrix (ld = nrows) and a FULL N x ncols copy
+ * of the vectors.  A step computes the rank's rows of the new iterate and its epilogue stores them into
+ * the local copy AND, over NVLink peer memory, into every other rank's copy -- the all-gather of the
+ * paper's HEMM ("gather") is fused into the kernel, tile by tile.  Only the FP64 tensor
+ * kernels take this path: CHASE_C128 with N % 8 == 0 and nrows % 8 == 0, CHASE_F64 with % 16
+ * (CHASE_ERR_ALIGN otherwise).  nranks <= CHASE_MAX_RANKS.
+ *
+ * chase_hemm_rows:  Y[rows, :] <- alpha (H_loc X - shift X[rows, :]) + beta Y[rows, :]  on this rank's
+ *   rows, X and Y full N x ncols DEVICE buffers (ld = N), X complete on entry.  peer_Y: HOST array of
+ *   npeers pointers valid ON THIS DEVICE to the other ranks' Y buffers (peer-mapped, e.g. through
+ *   chase_ipc_open); the rows are pushed to each.  npeers = 0 is a plain local row-block HEMM.
+ *   Asynchronous; no inter-GPU synchronisation (see chase_rows_barrier).
+ *
+ * chase_rows_barrier: all ranks' work enqueued so far on their streams has completed, including its
+ *   peer stores.  flags: this rank's DEVICE uint32[nranks], zeroed once by the caller; peer_flags: HOST
+ *   array [nranks] of pointers valid on this device to every rank's flags array (entry [rank] = flags);
+ *   seq: value strictly larger than any used before on these flags (same on all ranks).  Enqueues a
+ *   signal kernel (system-scope release stores of seq into flags[rank] of every rank) and a wait
+ *   kernel (spins, bounded to ~30 s, until all nranks entries of the local flags reach seq).
+ *
+ * chase_filter_rows_ws: the filter of chase_filter_ws on a row-sharded H: per degree step one
+ *   chase_hemm_rows launch on the active suffix and one chase_rows_barrier.  V (in: V_0 complete on
+ *   every rank; out: result complete on every rank) and workspace as in chase_filter_ws; peer_V /
+ *   peer_W: HOST arrays [nranks] of peer-mapped pointers to every rank's V / workspace (entry [rank]
+ *   ignored); *seq (HOST, in/out) carries the barrier sequence across calls (start at 0).
+ *   flags == NULL skips the barriers (single rank, or a caller that serialises the ranks itself). */
+int chase_hemm_rows(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, const void *X, void *Y,
+                    int64_t ncols, double alpha, double beta, double shift, chase_dtype_t dtype,
+                    int32_t npeers, void *const *peer_Y, void *stream);
+int chase_rows_barrier(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank,
+                       uint32_t seq, void *stream);
+int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
+                         const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
+                         void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
+                         void *const *peer_V, void *const *peer_W, uint32_t *flags,
+                         uint32_t *const *peer_flags, uint32_t *seq, void *stream);
+
+/* CUDA IPC plumbing for the peer pointers above (one process per GPU).  chase_ipc_export: handle
+ * (HOST, 64 bytes) of the allocation containing dev_ptr and dev_ptr's byte offset inside it.
+ * chase_ipc_open: maps a handle received from another process, enabling peer access; *base_out is
+ * the mapped allocation base (pass it to chase_ipc_close), the usable pointer is base + offset. */
+int chase_ipc_export(const void *dev_ptr, void *handle64, int64_t *offset);
+int chase_ipc_open(const void *handle64, void **base_out);
+int chase_ipc_close(void *base);
 
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
  * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with

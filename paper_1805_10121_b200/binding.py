@@ -23,6 +23,8 @@ EXPORTS = [
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
     "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_tiling",
     "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates",
+    "chase_hemm_rows", "chase_rows_barrier", "chase_filter_rows_ws", "chase_ipc_export", "chase_ipc_open",
+    "chase_ipc_close",
 ]
 
 _lib = None
@@ -85,6 +87,19 @@ def load() -> ctypes.CDLL:
     lib.chase_lanczos.argtypes = [vp, i64, vp, i64, i32, ctypes.c_int, vp, vp, vp, sz, vp]
     lib.chase_spectral_estimates.restype = ctypes.c_int
     lib.chase_spectral_estimates.argtypes = [i32, i64, vp, vp, i64, dbl, dbl, vp, vp, vp]
+    lib.chase_hemm_rows.restype = ctypes.c_int
+    lib.chase_hemm_rows.argtypes = [vp, i64, i64, i64, vp, vp, i64, dbl, dbl, dbl, ctypes.c_int, i32, vp, vp]
+    lib.chase_rows_barrier.restype = ctypes.c_int
+    lib.chase_rows_barrier.argtypes = [vp, vp, i32, i32, ctypes.c_uint32, vp]
+    lib.chase_filter_rows_ws.restype = ctypes.c_int
+    lib.chase_filter_rows_ws.argtypes = [vp, i64, i64, i64, vp, i64, vp, dbl, dbl, dbl, ctypes.c_int, vp, sz,
+                                         i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.chase_ipc_export.restype = ctypes.c_int
+    lib.chase_ipc_export.argtypes = [vp, vp, vp]
+    lib.chase_ipc_open.restype = ctypes.c_int
+    lib.chase_ipc_open.argtypes = [vp, vp]
+    lib.chase_ipc_close.restype = ctypes.c_int
+    lib.chase_ipc_close.argtypes = [vp]
     lib.chase_filter_strerror.restype = ctypes.c_char_p
     lib.chase_filter_strerror.argtypes = [ctypes.c_int]
     _lib = lib
@@ -336,3 +351,99 @@ def chase_spectral_estimates(alpha, beta, N: int, nev_nex: float, sigma: float =
     _check(load().chase_spectral_estimates(int(k), int(nruns), a.ctypes.data, b.ctypes.data, int(N), float(nev_nex),
                                            float(sigma), base, base + 8, base + 16))
     return (out[0], None, None) if nruns == 1 else (out[0], out[1], out[2])
+
+
+# ---------------------------------------------------------------------------------------------
+# Row-sharded path (one process per GPU; H row block per rank, fused NVLink all-gather)
+# ---------------------------------------------------------------------------------------------
+def _ptr_array(ptrs: Sequence[int]):
+    arr = (ctypes.c_void_p * max(len(ptrs), 1))()
+    for i, p in enumerate(ptrs):
+        arr[i] = int(p) if p else None
+    return arr
+
+
+def _check_rows(H_loc: torch.Tensor, N: int, row0: int):
+    if not H_loc.is_cuda or H_loc.dtype not in _DTYPE_CODE:
+        raise ValueError("H_loc must be a CUDA tensor of a supported dtype (there is no CPU path)")
+    _check_colmajor(H_loc, "H_loc")
+    nrows = H_loc.shape[0]
+    if H_loc.shape[1] != N or row0 < 0 or row0 + nrows > N:
+        raise ValueError("H_loc must be the nrows x N row block [row0, row0 + nrows) of H")
+    return nrows
+
+
+def chase_hemm_rows(H_loc: torch.Tensor, row0: int, X: torch.Tensor, Y: torch.Tensor, alpha: float = 1.0,
+                    beta: float = 0.0, shift: float = 0.0, peer_Y: Sequence[int] = (),
+                    stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """Y[rows] <- alpha (H_loc X - shift X[rows]) + beta Y[rows]; the rows are also stored through the
+    peer-mapped device pointers `peer_Y` (other ranks' Y buffers)."""
+    N, ncols = X.shape
+    nrows = _check_rows(H_loc, N, row0)
+    if not (X.is_cuda and Y.is_cuda) or X.dtype != H_loc.dtype or Y.dtype != H_loc.dtype or Y.shape != X.shape:
+        raise ValueError("X, Y must be CUDA tensors of H_loc's dtype and equal shape")
+    _check_colmajor(X, "X")
+    _check_colmajor(Y, "Y")
+    arr = _ptr_array(peer_Y)
+    with torch.cuda.device(H_loc.device):
+        _check(load().chase_hemm_rows(H_loc.data_ptr(), N, int(row0), nrows, X.data_ptr(), Y.data_ptr(), ncols,
+                                      float(alpha), float(beta), float(shift), _DTYPE_CODE[H_loc.dtype],
+                                      len(peer_Y), arr, _stream_ptr(stream)))
+    return Y
+
+
+def chase_rows_barrier(flags: torch.Tensor, peer_flags: Sequence[int], rank: int, seq: int,
+                       stream: Optional[torch.cuda.Stream] = None) -> None:
+    """Inter-GPU barrier on `stream` over flag arrays in peer memory (see include/chase_filter.h)."""
+    if not flags.is_cuda or flags.dtype != torch.int32 or flags.numel() < len(peer_flags):
+        raise ValueError("flags must be a CUDA int32 tensor with one entry per rank")
+    arr = _ptr_array(peer_flags)
+    with torch.cuda.device(flags.device):
+        _check(load().chase_rows_barrier(flags.data_ptr(), arr, len(peer_flags), int(rank), int(seq) & 0xFFFFFFFF,
+                                         _stream_ptr(stream)))
+
+
+def chase_filter_rows_ws(H_loc: torch.Tensor, row0: int, V: torch.Tensor, degrees, a: float, b: float,
+                         lambda1: float, workspace: torch.Tensor, rank: int = 0, peer_V: Sequence[int] = (),
+                         peer_W: Sequence[int] = (), flags: Optional[torch.Tensor] = None,
+                         peer_flags: Sequence[int] = (), seq: int = 0,
+                         stream: Optional[torch.cuda.Stream] = None) -> int:
+    """Row-sharded filter; peer_V / peer_W / peer_flags hold one device pointer per rank (own entry
+    ignored).  Returns the advanced barrier sequence number."""
+    N, ncols = V.shape
+    nrows = _check_rows(H_loc, N, row0)
+    if not V.is_cuda or V.dtype != H_loc.dtype:
+        raise ValueError("V must be a CUDA tensor of H_loc's dtype")
+    _check_colmajor(V, "V")
+    deg = _degrees_array(degrees, ncols)
+    nranks = max(len(peer_V), 1)
+    seq_c = ctypes.c_uint32(int(seq) & 0xFFFFFFFF)
+    with torch.cuda.device(H_loc.device):
+        _check(load().chase_filter_rows_ws(
+            H_loc.data_ptr(), N, int(row0), nrows, V.data_ptr(), ncols, deg.ctypes.data, float(a), float(b),
+            float(lambda1), _DTYPE_CODE[H_loc.dtype], workspace.data_ptr(),
+            workspace.numel() * workspace.element_size(), nranks, int(rank),
+            _ptr_array(peer_V) if len(peer_V) else None, _ptr_array(peer_W) if len(peer_W) else None,
+            flags.data_ptr() if flags is not None else None,
+            _ptr_array(peer_flags) if len(peer_flags) else None, ctypes.addressof(seq_c), _stream_ptr(stream)))
+    return int(seq_c.value)
+
+
+def chase_ipc_export(t: torch.Tensor):
+    """(64-byte handle, byte offset) of the CUDA allocation holding tensor `t` (for another process)."""
+    h = ctypes.create_string_buffer(64)
+    off = ctypes.c_int64()
+    with torch.cuda.device(t.device):
+        _check(load().chase_ipc_export(t.data_ptr(), h, ctypes.addressof(off)))
+    return bytes(h.raw), int(off.value)
+
+
+def chase_ipc_open(handle: bytes) -> int:
+    """Maps a handle exported by another process on the current device; returns the base pointer."""
+    base = ctypes.c_void_p()
+    _check(load().chase_ipc_open(ctypes.c_char_p(handle), ctypes.addressof(base)))
+    return int(base.value)
+
+
+def chase_ipc_close(base: int) -> None:
+    _check(load().chase_ipc_close(ctypes.c_void_p(base)))

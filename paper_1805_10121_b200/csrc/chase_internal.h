@@ -33,8 +33,11 @@ struct DmmaPlan {
     alignas(64) unsigned char tmap_B[2][128];   // [0]: buffer V, [1]: buffer W
     chase_dtype_t dtype;
     int64_t N, ncols;
+    int64_t M, row0;                            // row block of H this rank owns (M = N, row0 = 0 unless row-sharded)
     const void *H;
     void *buf[2];
+    int npeers;                                 // row-sharded: peer-mapped copies of buf[0], buf[1] on the other GPUs
+    void *peer_buf[2][CHASE_MAX_RANKS - 1];
 };
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
 // Column tiling one launch on `n` active columns would use on `sms` SMs:
@@ -44,6 +47,9 @@ void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_
 // only if the failure is "driver entry point unavailable"; anything else is reported).
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N,
                              void *V, void *W, int64_t ncols);
+// Row-sharded variant: H_loc is the nrows x N row block [row0, row0 + nrows) of H, column-major, ld = nrows.
+cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const void *H_loc, int64_t N, int64_t row0,
+                                  int64_t nrows, void *V, void *W, int64_t ncols);
 // Step reading buffer `src` (0/1) and writing buffer 1-src, active columns [s, ncols).
 cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
                              double c, int use_beta, cudaStream_t stream, const double *c_col = nullptr);

@@ -101,10 +101,15 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 }
 
 // ---------------------------------------------------------------- the kernel
+constexpr int kMaxPeers = CHASE_MAX_RANKS - 1;
 struct StepParams {
     const double *X;     // source iterate V_k, first ACTIVE column (ld = N elements)
     double *Y;           // destination (holds V_{k-1}, becomes V_{k+1}), first active column
-    int64_t N;           // matrix order
+    int64_t N;           // matrix order = length of k = leading dimension of X, Y
+    int64_t M;           // rows of H this launch owns (N unless row-sharded); H tile rows are local
+    int64_t row0;        // global index of local row 0 (rows of X, Y touched by the epilogue: row0 + local)
+    int npeers;          // row-sharded runs: the new rows are also stored into each peer GPU's copy of Y
+    double *peer_Y[kMaxPeers];   // peer-mapped pointers, already offset to the first active column
     int n;               // active columns
     int col0;            // first active column in the full buffer (TMA coordinate offset)
     int tiles_m;
@@ -337,8 +342,8 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                 int row;
                 if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
                 else row = m0 + wm * C::WM + (i >> 1) * 16 + (i & 1) * 8 + g;
-                if (row >= p.N) continue;
-                const int64_t off = ((int64_t)col * p.N + row) * NC;
+                if (row >= p.M) continue;
+                const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
                 if (CPLX) {
                     const double2 x = *reinterpret_cast<const double2 *>(p.X + off);
                     double2 y;
@@ -350,10 +355,13 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                         y.y = fma(beta, o.y, y.y);
                     }
                     *reinterpret_cast<double2 *>(p.Y + off) = y;
+                    for (int q = 0; q < p.npeers; ++q)      // fused all-gather: push the row block over NVLink
+                        *reinterpret_cast<double2 *>(p.peer_Y[q] + off) = y;
                 } else {
                     double y = alpha * (acc[0][i][j][e] - c * p.X[off]);
                     if (p.use_beta) y = fma(beta, p.Y[off], y);
                     p.Y[off] = y;
+                    for (int q = 0; q < p.npeers; ++q) p.peer_Y[q][off] = y;
                 }
             }
         }
@@ -397,9 +405,10 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return cudaErrorNotSupported;
     const cuuint64_t N = (cuuint64_t)plan->N;
-    {   // A: H viewed as (16 doubles, k, m_group)
-        cuuint64_t dims[3] = {16, N, N / C::ROWS128};
-        cuuint64_t strides[2] = {N * C::ESZ, 128};
+    {   // A: H (M x N, ld = M) viewed as (16 doubles, k, m_group)
+        const cuuint64_t M = (cuuint64_t)plan->M;
+        cuuint64_t dims[3] = {16, N, M / C::ROWS128};
+        cuuint64_t strides[2] = {M * C::ESZ, 128};
         cuuint32_t box[3] = {16, (cuuint32_t)C::BK, (cuuint32_t)(C::BM / C::ROWS128)};
         cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = enc((CUtensorMap *)plan->tmap_H, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)plan->H, dims,
@@ -502,9 +511,14 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     p.X = (const double *)plan->buf[src] + (size_t)s * col_doubles;
     p.Y = (double *)plan->buf[src ^ 1] + (size_t)s * col_doubles;
     p.N = plan->N;
+    p.M = plan->M;
+    p.row0 = plan->row0;
+    p.npeers = plan->npeers;
+    for (int q = 0; q < plan->npeers; ++q)
+        p.peer_Y[q] = (double *)plan->peer_buf[src ^ 1][q] + (size_t)s * col_doubles;
     p.n = (int)n;
     p.col0 = (int)s;
-    p.tiles_m = (int)((plan->N + C::BM - 1) / C::BM);
+    p.tiles_m = (int)((plan->M + C::BM - 1) / C::BM);
     choose_tiling<CPLX>(n, p.tiles_m, sm_count(), p.tiles_wide, p.tiles_narrow, p.narrow_w);
     p.alpha = alpha;
     p.beta = beta;
@@ -537,10 +551,18 @@ bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
 
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V, void *W,
                              int64_t ncols) {
+    return dmma_plan_create_rows(plan, dtype, H, N, 0, N, V, W, ncols);
+}
+
+cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const void *H_loc, int64_t N, int64_t row0,
+                                  int64_t nrows, void *V, void *W, int64_t ncols) {
     plan->dtype = dtype;
     plan->N = N;
+    plan->M = nrows;
+    plan->row0 = row0;
+    plan->npeers = 0;
     plan->ncols = ncols;
-    plan->H = H;
+    plan->H = H_loc;
     plan->buf[0] = V;
     plan->buf[1] = W;
     return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);

@@ -1,0 +1,113 @@
+"""Row-sharded path on ONE GPU (SURVEY 8(e) option 2).  The P "ranks" are logical: each has its own row
+block of H and its own full copies of the vector buffers on the same device, the peer pointers are
+simply the other copies' addresses, and the ranks' launches are issued one after the other on one
+stream (stream order stands in for the inter-GPU barrier; no kernel waits on another).  This checks
+what the kernel does with row offsets, the rectangular H view and the peer stores; the flag barrier is
+exercised with a single rank only."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_1805_10121_b200 as pkg
+from paper_1805_10121_b200 import sharding
+from paper_1805_10121_b200 import workloads as W
+from cheb_closed_form import rel_fro
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _dev(x):
+    out = W.empty_colmajor(x.shape[0], x.shape[1], x.dtype, DEV)
+    out.copy_(x)
+    return out
+
+
+def _row_blocks(H, world, align):
+    parts = sharding.row_partition(H.shape[0], world, align)
+    return parts, [_dev(H[r0:r0 + n, :]) for r0, n in parts]
+
+
+@pytest.mark.parametrize("dtype,N,n,world,align", [(torch.complex128, 520, 77, 3, 128), (torch.float64, 1040, 150, 2, 128),
+                                                    (torch.complex128, 776, 40, 4, 8), (torch.float64, 528, 33, 3, 16)])
+def test_hemm_rows_with_peer_pushes(dtype, N, n, world, align):
+    H = W.hermitian_gaussian_ensemble(N, dtype, seed=81)
+    X = W.gaussian_colmajor(N, n, dtype, seed=82)
+    Y = W.gaussian_colmajor(N, n, dtype, seed=83)
+    parts, Hb = _row_blocks(H, world, align)
+    Xs = [_dev(X) for _ in range(world)]
+    Ys = [_dev(Y) for _ in range(world)]
+    for r, (row0, nrows) in enumerate(parts):
+        peers = [Ys[q].data_ptr() for q in range(world) if q != r]
+        pkg.chase_hemm_rows(Hb[r], row0, Xs[r], Ys[r], alpha=0.7, beta=-1.3, shift=0.25, peer_Y=peers)
+    torch.cuda.synchronize()
+    ref = oracle.hemm(H.numpy(), X.numpy(), Y.numpy(), 0.7, -1.3, 0.25)
+    for q in range(world):
+        assert rel_fro(Ys[q].cpu().numpy(), ref) <= 1e-12, q
+
+
+@pytest.mark.parametrize("dtype,N,n,world", [(torch.complex128, 520, 77, 3), (torch.float64, 1040, 150, 2)])
+def test_filter_emulated_ranks_step_by_step(dtype, N, n, world):
+    """Alg. 4 driven from the host plan (chase_filter_scalars / _schedule) with one chase_hemm_rows per
+    rank and step on the active suffix; every rank's copy of V must end up equal to the oracle."""
+    w = W.make_config(2, N=N, ncols=n, dtype=dtype)
+    deg = w.degrees.numpy()
+    parts, Hb = _row_blocks(w.H, world, 128)
+    buf = [[_dev(w.V0) for _ in range(world)], [_dev(torch.zeros_like(w.V0)) for _ in range(world)]]
+    m_max, offset = pkg.chase_filter_schedule(deg)
+    alpha, beta, c = pkg.chase_filter_scalars(w.a, w.b, w.lambda1, m_max)
+    for k in range(1, m_max + 1):
+        s, src = int(offset[k]), (k - 1) & 1
+        for r, (row0, _) in enumerate(parts):
+            X, Y = buf[src][r][:, s:], buf[src ^ 1][r][:, s:]
+            peers = [buf[src ^ 1][q][:, s:].data_ptr() for q in range(world) if q != r]
+            pkg.chase_hemm_rows(Hb[r], row0, X, Y, alpha=alpha[k], beta=beta[k] if k > 1 else 0.0, shift=c, peer_Y=peers)
+    torch.cuda.synchronize()
+    ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), deg, w.a, w.b, w.lambda1)
+    assert np.all(deg % 2 == 0)                      # even degrees: the result sits in buffer 0
+    for q in range(world):
+        assert rel_fro(buf[0][q].cpu().numpy(), ref) <= 1e-12, q
+
+
+@pytest.mark.parametrize("with_flags", [False, True])
+def test_filter_rows_single_rank_equals_plain_filter(with_flags):
+    w = W.make_config(4, N=776, ncols=130)
+    H = _dev(w.H)
+    V1, V2 = _dev(w.V0), _dev(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=DEV)
+    pkg.chase_filter_ws(H, V1, w.degrees, w.a, w.b, w.lambda1, ws)
+    flags = torch.zeros(1, dtype=torch.int32, device=DEV) if with_flags else None
+    seq = pkg.chase_filter_rows_ws(H, 0, V2, w.degrees, w.a, w.b, w.lambda1, ws, rank=0,
+                                   flags=flags, peer_flags=[flags.data_ptr()] if with_flags else [], seq=5)
+    torch.cuda.synchronize()
+    assert torch.equal(V1, V2)
+    if with_flags:
+        m_max = int(w.degrees.max())
+        assert seq == 5 + 1 + m_max and int(flags.cpu()[0]) == seq      # one barrier on entry, one per step
+
+
+def test_rows_rejects_unsupported_layouts():
+    H = _dev(W.hermitian_gaussian_ensemble(64, torch.complex64, seed=1))
+    X = _dev(W.gaussian_colmajor(64, 4, torch.complex64, seed=2))
+    with pytest.raises(pkg.ChaseFilterError) as e:
+        pkg.chase_hemm_rows(H, 0, X, X.clone())
+    assert e.value.code == -6
+    H = _dev(W.hermitian_gaussian_ensemble(520, torch.complex128, seed=1))
+    X = _dev(W.gaussian_colmajor(520, 4, torch.complex128, seed=2))
+    with pytest.raises(pkg.ChaseFilterError) as e:       # 100 rows: not a multiple of 8
+        pkg.chase_hemm_rows(W.as_colmajor(H[:100, :]), 0, X, X.clone())
+    assert e.value.code == -6
+
+
+def test_row_sharded_filter_class_single_rank():
+    """RowShardedFilter with world = 1 (no IPC): same result as the oracle, barrier sequence advances."""
+    w = W.make_config(2, N=520, ncols=40)
+    f = sharding.RowShardedFilter(_dev(w.H), 0, w.N, w.ncols, rank=0, world=1)
+    f.V.copy_(w.V0)
+    f.run(w.degrees, w.a, w.b, w.lambda1)
+    torch.cuda.synchronize()
+    ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), w.degrees.numpy(), w.a, w.b, w.lambda1)
+    assert rel_fro(f.V.cpu().numpy(), ref) <= 1e-12
+    assert f.seq == 1 + int(w.degrees.max())
+    f.close()
