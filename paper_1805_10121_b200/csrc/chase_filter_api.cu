@@ -138,6 +138,16 @@ int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t nc
                            double beta, double c, const double *c_col, int use_beta, chase_dtype_t dtype,
                            cudaStream_t stream) {
     const int path = chase_filter_kernel_path(N, ncols, dtype);
+    const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
+    // A few vectors: one streaming pass over H.  In FP64 the narrow-tile DMMA kernel is the faster
+    // streamer from 3 columns on (measured: c128, N = 40000, 5 columns: 4.1 vs 3.0 TB/s).
+    const bool fp64_tensor = path == 1 && ncols > 2;
+    if (ncols <= kSkinnyMaxCols && !fp64_tensor && !(force && force[0] == '1')) {
+        StepArgs sa;
+        sa.H = H; sa.X = X; sa.Y = Y; sa.N = N; sa.n = ncols;
+        sa.alpha = alpha; sa.beta = beta; sa.c = c; sa.c_col = c_col; sa.use_beta = use_beta;
+        return (int)launch_step_skinny(dtype, sa, stream);
+    }
     if (path == 1) {
         DmmaPlan plan;
         cudaError_t e = dmma_plan_create(&plan, dtype, H, N, const_cast<void *>(X), Y, ncols);

@@ -26,6 +26,11 @@ struct StepArgs {
 // Generic FMA kernels: any N, any n, all four dtypes.
 cudaError_t launch_step_generic(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
 
+// Tall-skinny streaming kernel (csrc/step_skinny.cu): 1..kSkinnyMaxCols columns, all dtypes, any N;
+// bound by one pass over H from HBM.  Uses that H is Hermitian.
+constexpr int kSkinnyMaxCols = 8;
+cudaError_t launch_step_skinny(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
+
 // TMA + DMMA tensor kernels (CHASE_C128 with N % 8 == 0, CHASE_F64 with N % 16 == 0).
 // A plan holds the three tensor maps (H, and both vector buffers) of one chase_filter call.
 struct DmmaPlan {

@@ -78,3 +78,25 @@ def test_gpu_residuals_of_exact_eigenpairs():
     Q = W.as_colmajor(w.eigvecs[:, :40].contiguous())
     r = pkg.chase_residuals(_dev(w.H), _dev(Q), w.eigvals[:40].numpy().astype(np.float64)).cpu().numpy()
     assert np.all(r < 1e-13)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64, torch.complex64, torch.complex128])
+@pytest.mark.parametrize("N,n", [(1040, 5), (203, 1), (777, 8), (1536, 3), (64, 7)])
+def test_gpu_skinny_hemm_and_residuals(dtype, N, n):
+    """1..8 columns take the streaming kernel (csrc/step_skinny.cu): all dtypes, odd N, a chunk tail,
+    beta = 0 must not read Y, per-column shifts (residuals)."""
+    tol = 1e-12 if dtype in (torch.complex128, torch.float64) else 2e-5
+    H = W.hermitian_gaussian_ensemble(N, dtype, seed=91)
+    X = W.gaussian_colmajor(N, n, dtype, seed=92)
+    Y = W.gaussian_colmajor(N, n, dtype, seed=93)
+    Hd, Xd, Yd = _dev(H), _dev(X), _dev(Y)
+    pkg.chase_hemm(Hd, Xd, Yd, alpha=0.7, beta=-1.3, shift=0.25)
+    assert rel_fro(Yd.cpu().numpy(), oracle.hemm(H.numpy(), X.numpy(), Y.numpy(), 0.7, -1.3, 0.25)) <= tol
+    Yd.fill_(float("nan"))
+    pkg.chase_hemm(Hd, Xd, Yd)
+    assert rel_fro(Yd.cpu().numpy(), oracle.hemm(H.numpy(), X.numpy(), None)) <= tol
+    ritz = np.linspace(-2, 2, n)
+    got = pkg.chase_residuals(Hd, Xd, ritz).cpu().numpy()
+    np.testing.assert_allclose(got, oracle.residuals(H.numpy(), X.numpy(), ritz), rtol=10 * tol)
+    assert torch.equal(Xd.cpu(), X) and torch.equal(Hd.cpu(), H)
