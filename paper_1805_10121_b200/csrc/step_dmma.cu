@@ -17,7 +17,7 @@
 //   B (X tile, K-major as stored): row index = kgroup * BN + n, the 128B hold 8 (16) consecutive k.
 // The k index each MMA lane slot consumes is a free permutation; it is chosen so that every
 // fragment load is bank-conflict free under the swizzle (complex: k = 8q + 2t + a; real:
-// k = {0,3,12,15}[t] ^ {0,1,4,5}[a]), identically for A and B.
+// k = {0,10,4,14}[t] ^ a with 16-byte loads shared by two MMAs), identically for A and B.
 #include <cuda.h>
 
 #include <algorithm>
@@ -49,8 +49,12 @@ struct Cfg<false> {  // float64: CTA tile 128 x 128, warp tile 64 x 32 (2 x 4 wa
     static constexpr int BM = 128, BN = 128, WM = 64, WN = 32, WARPS_M = 2;
     static constexpr int ROWS128 = 16;
     static constexpr int ESZ = 8;
-    static constexpr int BK = 32;           // 64 KB / stage: same DMMA count per stage as complex
-    static constexpr int STAGES = 3;
+#ifndef F64_BK
+#define F64_BK 32
+#define F64_STAGES 3
+#endif
+    static constexpr int BK = F64_BK;       // 32: 64 KB / stage, same DMMA count per stage as complex
+    static constexpr int STAGES = F64_STAGES;
     static constexpr int GROUP_N = 12;
 };
 
@@ -152,13 +156,16 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
     const int wm = warp % C::WARPS_M, wn = warp / C::WARPS_M;
 
     // float64: lane-dependent byte offsets of the fragment loads, hoisted out of the k loop.
-    // MMA a of a 16-k group consumes, in lane slot t, k = {0,3,12,15}[t] ^ {0,1,4,5}[a] (conflict-free).
-    int real_a_off[4], real_b_off[4];
+    // MMA a of a 16-k group consumes, in lane slot t, k = {0,10,4,14}[t] ^ a.  One 16-byte load of A
+    // yields matrix rows 2g and 2g+1 (the lane's "row g" of an even and an odd 8-row block), one 16-byte
+    // load of B yields k and k^1, i.e. the operands of MMAs a and a^1: 24 LDS.128 per 128 MMAs, every
+    // one conflict-free under the swizzle (k bits (1,2) and (2,3) both take 4 distinct values over t).
+    int real_a_off[4], real_b_off[2];
 #pragma unroll
     for (int a = 0; a < 4; ++a) {
-        const int kl = (3 * (t & 1) + 12 * (t >> 1)) ^ ((a & 1) | ((a & 2) << 1));
-        real_a_off[a] = kl * 128 + (((g >> 1) ^ (kl & 7)) << 4) + ((g & 1) << 3);     // row ml = g; ml = g+8: ^ 64
-        real_b_off[a] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4) + ((kl & 1) << 3);
+        const int kl = (10 * (t & 1) + 4 * (t >> 1)) ^ a;
+        real_a_off[a] = kl * 128 + ((g ^ (kl & 7)) << 4);
+        if ((a & 1) == 0) real_b_off[a >> 1] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4);
     }
 
     for (int kt = 0; kt < KT; ++kt) {
@@ -206,21 +213,32 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
 #pragma unroll
             for (int kq = 0; kq < BK / 16; ++kq) {
 #pragma unroll
-                for (int a = 0; a < 4; ++a) {
-                    double af[MB];
-#pragma unroll
-                    for (int i = 0; i < MB; ++i) {
-                        const int mg = wm * (C::WM / 16) + (i >> 1);
-                        af[i] = *reinterpret_cast<const double *>(
-                            sa + (mg * BK + kq * 16) * 128 + (real_a_off[a] ^ ((i & 1) << 6)));
-                    }
+                for (int ap = 0; ap < 2; ++ap) {          // MMAs a = 2 ap and 2 ap + 1 share their B loads
+                    double2 b2[NB];
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
                         if (!FULL && j >= jmax) break;
-                        const double b = *reinterpret_cast<const double *>(
-                            sb + (kq * BN + (j * WARPS_N + wn) * 8) * 128 + real_b_off[a]);
+                        b2[j] = *reinterpret_cast<const double2 *>(
+                            sb + (kq * BN + (j * WARPS_N + wn) * 8) * 128 + real_b_off[ap]);
+                    }
 #pragma unroll
-                        for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                    for (int a1 = 0; a1 < 2; ++a1) {
+                        double af[MB];
+#pragma unroll
+                        for (int i = 0; i < MB; i += 2) {
+                            const int mg = wm * (C::WM / 16) + (i >> 1);
+                            const double2 v = *reinterpret_cast<const double2 *>(
+                                sa + (mg * BK + kq * 16) * 128 + real_a_off[2 * ap + a1]);
+                            af[i] = v.x;          // matrix row 2g     of the 16-row group
+                            af[i + 1] = v.y;      // matrix row 2g + 1
+                        }
+#pragma unroll
+                        for (int j = 0; j < NB; ++j) {
+                            if (!FULL && j >= jmax) break;
+                            const double b = a1 ? b2[j].y : b2[j].x;
+#pragma unroll
+                            for (int i = 0; i < MB; ++i) dmma884(acc[0][i][j][0], acc[0][i][j][1], af[i], b);
+                        }
                     }
                 }
             }
@@ -341,7 +359,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
             for (int i = 0; i < MB; ++i) {
                 int row;
                 if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
-                else row = m0 + wm * C::WM + (i >> 1) * 16 + (i & 1) * 8 + g;
+                else row = m0 + wm * C::WM + (i >> 1) * 16 + 2 * g + (i & 1);
                 if (row >= p.M) continue;
                 const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
                 if (CPLX) {
