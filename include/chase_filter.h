@@ -89,8 +89,10 @@ int chase_filter(const void *H, int64_t N, void *V, int64_t ncols, const int32_t
                  double a, double b, double lambda1, chase_dtype_t dtype, void *stream);
 
 /* End-to-end convenience for callers whose data lives on the HOST: H and V are HOST
- * pointers (pinned or pageable).  Allocates device buffers, copies H and V to the device,
- * runs chase_filter_ws, copies V back, frees, and SYNCHRONISES before returning.
+ * pointers (pinned or pageable).  Allocates device buffers, copies V and H to the device,
+ * runs the filter, copies V back, frees, and SYNCHRONISES before returning.  On the FP64 tensor
+ * path H is uploaded in 8 row panels on a second stream and the first degree step runs panel by
+ * panel as the rows arrive, so the upload of H hides behind that step.
  * `device` is the CUDA device ordinal. */
 int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols,
                       const int32_t *degrees, double a, double b, double lambda1,

@@ -292,9 +292,33 @@ int chase_filter_step_tiling(int64_t N, int64_t n_active, chase_dtype_t dtype, i
     return CHASE_OK;
 }
 
+}  // extern "C"
+
+namespace chase {
+// H (device) is still empty on entry: it is filled from H_host panel by panel on copy_stream while the
+// first step already runs on the panels that have arrived (chase_filter_host).
+struct HostUpload {
+    const void *H_host;
+    cudaStream_t copy_stream;
+};
+static int filter_impl(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                       double a, double b, double lambda1, chase_dtype_t dtype,
+                       void *workspace, size_t workspace_bytes, void *stream_, const HostUpload *up);
+}  // namespace chase
+
+extern "C" {
+
 int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                     double a, double b, double lambda1, chase_dtype_t dtype,
                     void *workspace, size_t workspace_bytes, void *stream_) {
+    return filter_impl(H, N, V, ncols, degrees, a, b, lambda1, dtype, workspace, workspace_bytes, stream_, nullptr);
+}
+
+}  // extern "C"
+
+static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
+                              double a, double b, double lambda1, chase_dtype_t dtype,
+                              void *workspace, size_t workspace_bytes, void *stream_, const HostUpload *up) {
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t w = elem_bytes(dtype);
     if (w == 0) return CHASE_ERR_DTYPE;
@@ -336,10 +360,44 @@ int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int3
         if (e != cudaSuccess) return (int)e;
     }
 
+    if (up && !use_dmma) {   // no panel-wise first step on this kernel family: plain upload, then the usual loop
+        cudaError_t e = cudaMemcpyAsync(const_cast<void *>(H), up->H_host, (size_t)N * (size_t)N * w,
+                                        cudaMemcpyHostToDevice, stream);
+        if (e != cudaSuccess) return (int)e;
+    }
     for (int k = 1; k <= m_max; ++k) {
         const int64_t s = offset[k];
         const int src = (k - 1) & 1;
         cudaError_t e;
+        if (use_dmma && k == 1 && up) {
+            // Step 1 row panel by row panel, each as soon as its rows of H have landed: the upload of H
+            // (26 GB at cfg 4, ~0.5 s over PCIe) hides behind the first step (~0.7 s).
+            const int64_t tiles = (N + 127) / 128;
+            const int panels = (int)std::min<int64_t>(8, tiles);
+            const int64_t rows_per = (tiles + panels - 1) / panels * 128;
+            std::vector<cudaEvent_t> ev;
+            for (int64_t r0 = 0; r0 < N; r0 += rows_per) {
+                const int64_t rows = std::min(rows_per, N - r0);
+                cudaEvent_t evp;
+                if ((e = cudaEventCreateWithFlags(&evp, cudaEventDisableTiming)) != cudaSuccess) return (int)e;
+                ev.push_back(evp);
+                e = cudaMemcpy2DAsync((char *)const_cast<void *>(H) + (size_t)r0 * w, (size_t)N * w,
+                                      (const char *)up->H_host + (size_t)r0 * w, (size_t)N * w, (size_t)rows * w,
+                                      (size_t)N, cudaMemcpyHostToDevice, up->copy_stream);
+                if (e == cudaSuccess) e = cudaEventRecord(evp, up->copy_stream);
+                if (e != cudaSuccess) return (int)e;
+            }
+            int pi = 0;
+            for (int64_t r0 = 0; r0 < N; r0 += rows_per, ++pi) {
+                const int64_t rows = std::min(rows_per, N - r0);
+                DmmaPlan pp;
+                if ((e = cudaStreamWaitEvent(stream, ev[pi], 0)) != cudaSuccess) return (int)e;
+                if ((e = dmma_plan_create_panel(&pp, dtype, H, N, r0, rows, V, workspace, ncols)) != cudaSuccess) return (int)e;
+                if ((e = dmma_launch_step(&pp, src, s, alpha[k], beta[k], c, 0, stream)) != cudaSuccess) return (int)e;
+            }
+            for (cudaEvent_t evp : ev) cudaEventDestroy(evp);
+            continue;
+        }
         if (use_dmma) {
             e = dmma_launch_step(&plan, src, s, alpha[k], beta[k], c, k > 1, stream);
         } else if (use_tf32) {
@@ -374,6 +432,8 @@ int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int3
     }
     return CHASE_OK;
 }
+
+extern "C" {
 
 int chase_filter(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                  double a, double b, double lambda1, chase_dtype_t dtype, void *stream_) {
@@ -421,16 +481,24 @@ int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols
     if ((e = cudaMalloc(&dH, hb)) != cudaSuccess) fail(e);
     if (rc == CHASE_OK && (e = cudaMalloc(&dV, vb)) != cudaSuccess) fail(e);
     if (rc == CHASE_OK && (e = cudaMalloc(&dW, wb)) != cudaSuccess) fail(e);
+    cudaStream_t cp = nullptr;
+    if (rc == CHASE_OK && (e = cudaStreamCreateWithFlags(&cp, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
     if (rc == CHASE_OK && (e = cudaMemcpyAsync(dV, V_host, vb, cudaMemcpyHostToDevice, st)) != cudaSuccess) fail(e);
-    if (rc == CHASE_OK && (e = cudaMemcpyAsync(dH, H_host, hb, cudaMemcpyHostToDevice, st)) != cudaSuccess) fail(e);
-    if (rc == CHASE_OK)
-        rc = chase_filter_ws(dH, N, dV, ncols, degrees, a, b, lambda1, dtype, dW, wb, (void *)st);
+    if (rc == CHASE_OK) {   // H goes up inside the filter, overlapped with its first step
+        HostUpload up{H_host, cp};
+        rc = filter_impl(dH, N, dV, ncols, degrees, a, b, lambda1, dtype, dW, wb, (void *)st, &up);
+    }
+    (void)hb;
     if (rc == CHASE_OK && (e = cudaMemcpyAsync(V_host, dV, vb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) fail(e);
     e = cudaStreamSynchronize(st);
     if (rc == CHASE_OK && e != cudaSuccess) fail(e);
     cudaFree(dH);
     cudaFree(dV);
     cudaFree(dW);
+    if (cp) {
+        cudaStreamSynchronize(cp);
+        cudaStreamDestroy(cp);
+    }
     cudaStreamDestroy(st);
     return rc;
 }

@@ -38,7 +38,8 @@ struct DmmaPlan {
     alignas(64) unsigned char tmap_B[2][128];   // [0]: buffer V, [1]: buffer W
     chase_dtype_t dtype;
     int64_t N, ncols;
-    int64_t M, row0;                            // row block of H this rank owns (M = N, row0 = 0 unless row-sharded)
+    int64_t M, row0;                            // row block of H this launch owns (M = N, row0 = 0 unless row-sharded)
+    int64_t ldh;                                // leading dimension of the H view (M for a packed row block, N for a panel of the full H)
     const void *H;
     void *buf[2];
     int npeers;                                 // row-sharded: peer-mapped copies of buf[0], buf[1] on the other GPUs
@@ -55,6 +56,10 @@ cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H,
 // Row-sharded variant: H_loc is the nrows x N row block [row0, row0 + nrows) of H, column-major, ld = nrows.
 cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const void *H_loc, int64_t N, int64_t row0,
                                   int64_t nrows, void *V, void *W, int64_t ncols);
+// Row panel [row0, row0 + nrows) of the FULL N x N matrix (ld = N): used to start the first step while H is
+// still being uploaded panel by panel (chase_filter_host).
+cudaError_t dmma_plan_create_panel(DmmaPlan *plan, chase_dtype_t dtype, const void *H_full, int64_t N, int64_t row0,
+                                   int64_t nrows, void *V, void *W, int64_t ncols);
 // Step reading buffer `src` (0/1) and writing buffer 1-src, active columns [s, ncols).
 cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
                              double c, int use_beta, cudaStream_t stream, const double *c_col = nullptr);

@@ -426,7 +426,7 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     {   // A: H (M x N, ld = M) viewed as (16 doubles, k, m_group)
         const cuuint64_t M = (cuuint64_t)plan->M;
         cuuint64_t dims[3] = {16, N, M / C::ROWS128};
-        cuuint64_t strides[2] = {M * C::ESZ, 128};
+        cuuint64_t strides[2] = {(cuuint64_t)plan->ldh * C::ESZ, 128};
         cuuint32_t box[3] = {16, (cuuint32_t)C::BK, (cuuint32_t)(C::BM / C::ROWS128)};
         cuuint32_t estr[3] = {1, 1, 1};
         CUresult r = enc((CUtensorMap *)plan->tmap_H, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, (void *)plan->H, dims,
@@ -577,10 +577,27 @@ cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const voi
     plan->dtype = dtype;
     plan->N = N;
     plan->M = nrows;
+    plan->ldh = nrows;
     plan->row0 = row0;
     plan->npeers = 0;
     plan->ncols = ncols;
     plan->H = H_loc;
+    plan->buf[0] = V;
+    plan->buf[1] = W;
+    return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);
+}
+
+cudaError_t dmma_plan_create_panel(DmmaPlan *plan, chase_dtype_t dtype, const void *H_full, int64_t N, int64_t row0,
+                                   int64_t nrows, void *V, void *W, int64_t ncols) {
+    const size_t esz = dtype == CHASE_C128 ? 16 : 8;
+    plan->dtype = dtype;
+    plan->N = N;
+    plan->M = nrows;
+    plan->ldh = N;
+    plan->row0 = row0;
+    plan->npeers = 0;
+    plan->ncols = ncols;
+    plan->H = (const char *)H_full + (size_t)row0 * esz;
     plan->buf[0] = V;
     plan->buf[1] = W;
     return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);

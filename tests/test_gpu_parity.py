@@ -172,10 +172,19 @@ def test_p9_uniform_vs_mixed_on_gpu():
         assert rel_fro(gsub, got[:, cols]) <= 1e-13
 
 
-def test_host_entry_point():
-    w = W.make_config(2, N=256, ncols=24)
-    V = w.V0.clone()
-    V = W.as_colmajor(V)
+@pytest.mark.parametrize("cfg,N,ncols,dtype", [
+    (2, 256, 24, None),                  # c128, two row panels
+    (2, 520, 33, None),                  # c128, 5 panels, the last one 8 rows
+    (4, 2064, 70, None),                 # c128, 8 panels of 384 rows, ragged tail, degrees 8..36
+    (3, 1040, 50, None),                 # f64
+    (5, 768, 100, None),                 # c64: tensor path without panel-wise first step (plain upload)
+    (2, 203, 9, torch.complex128),       # odd N: generic kernels
+])
+def test_host_entry_point(cfg, N, ncols, dtype):
+    """chase_filter_host: host buffers in, host buffers out; H is uploaded panel by panel under the first
+    step on the FP64 tensor path."""
+    w = W.make_config(cfg, N=N, ncols=ncols, dtype=dtype)
+    V = W.as_colmajor(w.V0.clone())
     pkg.chase_filter_host(w.H, V, w.degrees, w.a, w.b, w.lambda1, device=0)
     assert_parity(V.numpy(), run_oracle(w), w.dtype)
 
