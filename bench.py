@@ -420,6 +420,26 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_aux:
         aux = time_aux_ops(pkg, w, V, device)
 
+    # ---- comparator (context, not a dependency): one full-width H @ V0 through torch.matmul = cuBLAS ------
+    comparator = None
+    if rank == 0 and world == 1 and not args.no_aux:
+        try:
+            f = 8.0 if dtype.is_complex else 2.0
+            out = torch.matmul(w.H, w.V0)          # warm-up (also picks the cuBLAS algorithm)
+            torch.cuda.synchronize()
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record()
+            out = torch.matmul(w.H, w.V0)
+            c1.record()
+            torch.cuda.synchronize()
+            ms = c0.elapsed_time(c1)
+            comparator = {"what": "torch.matmul(H, V0), all columns, no epilogue (cuBLAS GEMM on the same box)",
+                          "ms": ms, "gflops": f * N * N * n / ms * 1e-6,
+                          "ours_full_width_step_gflops": (aux or {}).get("chase_hemm", {}).get("gflops")}
+            del out
+        except RuntimeError as exc:                 # e.g. out of memory: context only
+            comparator = {"error": str(exc)[:200]}
+
     # ---- e2e: HOST buffers through chase_filter_host (H2D + filter + D2H inside the timed call) --
     e2e = None
     if not args.no_e2e:
@@ -449,7 +469,7 @@ def run_ours(args):
                                                                torch.float32: "f32"}[dtype],
             "data": "synthetic", "config": workload_config(args, w, world), "clocks": clocks,
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
-            "parity": parity, "aux_ops": aux, "wall_s_timed_region": t_wall,
+            "parity": parity, "aux_ops": aux, "comparator_cublas": comparator, "wall_s_timed_region": t_wall,
             "fraction_of_fp64_peak": roofline["frac"] if is_f64 else None,
         }
         print(json.dumps(line))
