@@ -49,9 +49,9 @@ extern "C" {
 
 typedef enum {
     CHASE_F32 = 0,  /* float,                 tcgen05 3xTF32 tensor path when N % 4 == 0, else FP32 FMA */
-    CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N % 16 == 0) */
+    CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N is even) */
     CHASE_C64 = 2,  /* interleaved float2,    tcgen05 3xTF32 tensor path when N % 2 == 0, else FP32 FMA */
-    CHASE_C128 = 3  /* interleaved double2,   FP64 (DMMA tensor path when N % 8 == 0) */
+    CHASE_C128 = 3  /* interleaved double2,   FP64 (DMMA tensor path for every N >= 16) */
 } chase_dtype_t;
 
 enum {
@@ -220,7 +220,7 @@ int chase_ipc_open(const void *handle64, void **base_out);
 int chase_ipc_close(void *base);
 
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
- * N % 8 == 0, f64 with N % 16 == 0), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
+ * any N >= 16, f64 with even N), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
  * N % 4 == 0; FP32 operands split on chip into two TF32 parts, FP32 accumulation), 0 = generic FMA
  * kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1 turns 2
  * into 0.  Negative = invalid arguments. */

@@ -31,7 +31,7 @@ cudaError_t launch_step_generic(chase_dtype_t dtype, const StepArgs &a, cudaStre
 constexpr int kSkinnyMaxCols = 8;
 cudaError_t launch_step_skinny(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
 
-// TMA + DMMA tensor kernels (CHASE_C128 with N % 8 == 0, CHASE_F64 with N % 16 == 0).
+// TMA + DMMA tensor kernels (CHASE_C128 with any N >= 16, CHASE_F64 with even N).
 // A plan holds the three tensor maps (H, and both vector buffers) of one chase_filter call.
 struct DmmaPlan {
     alignas(64) unsigned char tmap_H[128];
@@ -39,6 +39,7 @@ struct DmmaPlan {
     chase_dtype_t dtype;
     int64_t N, ncols;
     int64_t M, row0;                            // row block of H this launch owns (M = N, row0 = 0 unless row-sharded)
+    int a_2d;                                   // set by the plan: 2-D H view (M not a multiple of the 128-byte row group)
     int64_t ldh;                                // leading dimension of the H view (M for a packed row block, N for a panel of the full H)
     const void *H;
     void *buf[2];

@@ -112,6 +112,7 @@ struct StepParams {
     int64_t N;           // matrix order = length of k = leading dimension of X, Y
     int64_t M;           // rows of H this launch owns (N unless row-sharded); H tile rows are local
     int64_t row0;        // global index of local row 0 (rows of X, Y touched by the epilogue: row0 + local)
+    int a_2d;            // H view: 0 = one 3-D box per stage (M % ROWS128 == 0), 1 = BM / ROWS128 2-D boxes (any M)
     int npeers;          // row-sharded runs: the new rows are also stored into each peer GPU's copy of Y
     double *peer_Y[kMaxPeers];   // peer-mapped pointers, already offset to the first active column
     int n;               // active columns
@@ -308,8 +309,16 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                 const uint32_t sa = smem_base + s * S::STAGE_BYTES, sb = sa + S::A_BYTES;
                 mbar_expect_tx(full, S::STAGE_BYTES);
                 const int k0 = kt * BK;
-                // A: view (16 doubles, k, m_group); one box {16, BK, BM / ROWS128}
-                tma_load_3d(sa, &tmapA, full, 0, k0, m0 / C::ROWS128);
+                if (!p.a_2d) {
+                    // A: view (16 doubles, k, m_group); one box {16, BK, BM / ROWS128}
+                    tma_load_3d(sa, &tmapA, full, 0, k0, m0 / C::ROWS128);
+                } else {
+                    // A: view (doubles along m, k); one box {16, BK} per 128-byte row group -- the same
+                    // shared-memory image, rows past M zero-filled (any M, e.g. the paper's odd sizes)
+#pragma unroll 4
+                    for (int gI = 0; gI < BM / C::ROWS128; ++gI)
+                        tma_load_2d(sa + gI * BK * 128, &tmapA, full, (m0 + gI * C::ROWS128) * (CPLX ? 2 : 1), k0);
+                }
                 // B: (doubles along k, column); boxes {16 doubles, BN}
                 if (CPLX) {
                     tma_load_2d(sb, &tmapB, full, 2 * k0, p.col0 + n0);
@@ -423,7 +432,17 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     EncodeTiledFn enc = get_encode_fn();
     if (!enc) return cudaErrorNotSupported;
     const cuuint64_t N = (cuuint64_t)plan->N;
-    {   // A: H (M x N, ld = M) viewed as (16 doubles, k, m_group)
+    plan->a_2d = plan->M % C::ROWS128 != 0;
+    if (plan->a_2d) {   // A: H viewed as (doubles along m, k): 2-D, rows past M are out of bounds -> zero fill
+        cuuint64_t dims[2] = {(cuuint64_t)plan->M * (CPLX ? 2 : 1), N};
+        cuuint64_t strides[1] = {(cuuint64_t)plan->ldh * C::ESZ};
+        cuuint32_t box[2] = {16, (cuuint32_t)C::BK};
+        cuuint32_t estr[2] = {1, 1};
+        CUresult r = enc((CUtensorMap *)plan->tmap_H, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void *)plan->H, dims,
+                         strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+    } else {   // A: H (M x N, ld = ldh) viewed as (16 doubles, k, m_group)
         const cuuint64_t M = (cuuint64_t)plan->M;
         cuuint64_t dims[3] = {16, N, M / C::ROWS128};
         cuuint64_t strides[2] = {(cuuint64_t)plan->ldh * C::ESZ, 128};
@@ -531,6 +550,7 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     p.N = plan->N;
     p.M = plan->M;
     p.row0 = plan->row0;
+    p.a_2d = plan->a_2d;
     p.npeers = plan->npeers;
     for (int q = 0; q < plan->npeers; ++q)
         p.peer_Y[q] = (double *)plan->peer_buf[src ^ 1][q] + (size_t)s * col_doubles;
@@ -562,8 +582,8 @@ void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_
 
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     if (ncols < 1 || N < 16 || N > (1 << 28) || ncols > (1 << 28)) return false;
-    if (dtype == CHASE_C128) return N % 8 == 0;
-    if (dtype == CHASE_F64) return N % 16 == 0;
+    if (dtype == CHASE_C128) return true;           // column stride N * 16 bytes: always a TMA-legal stride
+    if (dtype == CHASE_F64) return N % 2 == 0;      // TMA strides must be multiples of 16 bytes
     return false;
 }
 

@@ -81,11 +81,32 @@ def test_reduced_configs(cfg, N, ncols):
 
 @pytest.mark.parametrize("dtype", [torch.float32, torch.float64, torch.complex64, torch.complex128])
 @pytest.mark.parametrize("N,ncols", [(61, 5), (203, 33), (257, 1)])
-def test_generic_shapes_all_dtypes(dtype, N, ncols):
-    """Sizes no TMA path accepts (odd N): the generic FMA kernels, all four dtypes."""
+def test_generic_shapes_all_dtypes(dtype, N, ncols, monkeypatch):
+    """The generic FMA kernels, all four dtypes, odd N (complex128 takes the tensor path for every N, so
+    it is forced onto the generic kernels here)."""
+    monkeypatch.setenv("CHASE_FILTER_FORCE_GENERIC", "1")
     w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
     assert pkg.chase_filter_kernel_path(N, ncols, dtype) == 0
     assert_parity(run_gpu(w), run_oracle(w), dtype)
+
+
+@pytest.mark.parametrize("dtype,N,ncols", [
+    (torch.complex128, 203, 33),     # odd N: 2-D TMA view of H, ragged row group, k tail
+    (torch.complex128, 1161, 70),    # odd N, several row tiles (9273 = 8 * 1161 + ... is the paper's NaCl size class)
+    (torch.complex128, 61, 5),
+    (torch.float64, 1042, 150),      # even N, not a multiple of 16
+    (torch.float64, 206, 20),
+])
+def test_tensor_path_takes_unaligned_N(dtype, N, ncols):
+    """The paper's own matrix sizes are odd (9273, 13379, 47349, 62681): the FP64
+    tensor kernels must take them (c128: any N; f64: even N)."""
+    w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
+    assert pkg.chase_filter_kernel_path(N, ncols, dtype) == 1
+    assert_parity(run_gpu(w), run_oracle(w), dtype)
+    # and through the host entry point (panel-wise upload with a ragged last panel)
+    V = W.as_colmajor(w.V0.clone())
+    pkg.chase_filter_host(w.H, V, w.degrees, w.a, w.b, w.lambda1, device=0)
+    assert_parity(V.numpy(), run_oracle(w), dtype)
 
 
 @pytest.mark.parametrize("dtype,N,ncols", [
