@@ -307,28 +307,41 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                 const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
                 const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
                 {
+                    // all loads of a tile first (independent, pipelined through the LSU), then the stores
+                    constexpr int NA = A_BYTES / 16 / CT;
+                    float4 va[NA];
 #pragma unroll
-                for (int i = 0; i < A_BYTES / 16 / CT; ++i) {
-                    const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                    sts128(sa_lo + off, split_lo(lds128(sa_hi + off)));
-                }
-                if (CPLX) {
+                    for (int i = 0; i < NA; ++i) va[i] = lds128(sa_hi + (uint32_t)(ct + i * CT) * 16);
+                    if (CPLX) {
+                        constexpr int NB = B_BYTES / 2 / 16 / CT;
+                        float4 vb[NB];
 #pragma unroll
-                    for (int i = 0; i < B_BYTES / 2 / 16 / CT; ++i) {
-                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                        const float4 v = lds128(sb_hi + off);
-                        const float4 lo = split_lo(v);
-                        sts128(sb_lo + off, lo);
-                        sts128(sb_hi + B_BYTES / 2 + off, rot_mi(v));
-                        sts128(sb_lo + B_BYTES / 2 + off, rot_mi(lo));
+                        for (int i = 0; i < NB; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
+#pragma unroll
+                        for (int i = 0; i < NB; ++i) {
+                            const uint32_t off = (uint32_t)(ct + i * CT) * 16;
+                            const float4 lo = split_lo(vb[i]);
+                            sts128(sb_lo + off, lo);
+                            sts128(sb_hi + B_BYTES / 2 + off, rot_mi(vb[i]));
+                            sts128(sb_lo + B_BYTES / 2 + off, rot_mi(lo));
+                        }
+                    } else {
+                        constexpr int NB = B_BYTES / 16 / CT;
+                        float4 vb[NB / 2];
+#pragma unroll
+                        for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
+#pragma unroll
+                        for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
+#pragma unroll
+                        for (int i = 0; i < NB / 2; ++i) sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, split_lo(vb[i]));
+#pragma unroll
+                        for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + (i + NB / 2) * CT) * 16);
+#pragma unroll
+                        for (int i = 0; i < NB / 2; ++i)
+                            sts128(sb_lo + (uint32_t)(ct + (i + NB / 2) * CT) * 16, split_lo(vb[i]));
                     }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < B_BYTES / 16 / CT; ++i) {
-                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                        sts128(sb_lo + off, split_lo(lds128(sb_hi + off)));
-                    }
-                }
                 }
                 // generic-proxy writes -> visible to the tensor core's async-proxy reads
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
