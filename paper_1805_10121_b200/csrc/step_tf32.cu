@@ -441,14 +441,10 @@ cudaError_t encode_kmajor(CUtensorMap *map, const void *base, int64_t KF, int64_
 }
 
 int sm_count() {
-    static int sms = 0;
-    static std::once_flag once;
-    std::call_once(once, [] {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-            sms = 148;
-    });
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
+        sms = 148;
     return sms;
 }
 
@@ -526,15 +522,21 @@ cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H,
 }
 
 void *tf32_shared_sync_counter() {
-    static void *buf = nullptr;
-    static std::once_flag once;
-    std::call_once(once, [] {
-        if (cudaMalloc(&buf, 256) != cudaSuccess) {
-            buf = nullptr;
+    // one small buffer per device (a process may drive several GPUs), allocated on first use
+    static std::mutex mu;
+    static void *buf[64] = {};
+    static bool tried[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!tried[dev]) {
+        tried[dev] = true;
+        if (cudaMalloc(&buf[dev], 256) != cudaSuccess) {
+            buf[dev] = nullptr;
             (void)cudaGetLastError();
         }
-    });
-    return buf;
+    }
+    return buf[dev];
 }
 
 cudaError_t tf32_launch_step(const Tf32Plan *plan, int src, int64_t s, double alpha, double beta, double c,
