@@ -20,7 +20,9 @@
  *
  * Layouts (Listing 2): all matrices COLUMN-MAJOR, leading dimension N;
  * complex = interleaved (re, im) like std::complex<T>.  H is N x N, FULL Hermitian storage
- * (both triangles; read as a general matrix), never written.  V is N x ncols.
+ * (both triangles), EXACTLY Hermitian (H[i,j] == conj(H[j,i]) bitwise, real diagonal): a kernel may
+ * read an entry from either triangle (the tcgen05 and streaming kernels read row m as the conjugate
+ * of the contiguous column m).  H is never written.  V is N x ncols.
  *
  * Degrees: any m_j >= 0, non-decreasing.  0 leaves the column untouched, odd values are
  * accepted (the paper emits even ones only so that the result lands in V without a copy,
