@@ -145,3 +145,61 @@ def test_step_tiling_shortens_the_tail_of_the_metric_config():
     """cfg 4 full width: 2000 = 31 x 64 + 16 columns; the ragged 16 columns must not cost a full tile."""
     tm, tw, tn, nw = pkg.chase_filter_step_tiling(40000, 2000, torch.complex128, 148)
     assert (tm, tw) == (313, 31) and tn * nw >= 16 and nw < 64
+
+
+def test_rows_and_lanczos_validation_rejects_before_any_launch():
+    """chase_hemm_rows / chase_filter_rows_ws / chase_rows_barrier / chase_lanczos: fake pointers, every call
+    must come back with its error code before touching CUDA."""
+    import ctypes as C
+    lib = pkg.load()
+    before = pkg.chase_filter_launch_count()
+    H, X, Y = 0x1000, 0x2000, 0x3000
+    peers = (C.c_void_p * 2)(0x4000, 0x5000)
+
+    def hemm_rows(N=64, row0=0, nrows=32, ncols=4, dtype=3, npeers=0, peer=None, x=X, y=Y, alpha=1.0):
+        return lib.chase_hemm_rows(H, N, row0, nrows, x, y, ncols, alpha, 0.0, 0.0, dtype, npeers, peer, None)
+
+    assert hemm_rows(dtype=9) == -4
+    assert hemm_rows(dtype=2) == -6                       # only the FP64 tensor kernels take row blocks
+    assert hemm_rows(nrows=12) == -6                      # not a multiple of the 8-row group
+    assert hemm_rows(row0=40, nrows=32) == -1             # block leaves the matrix
+    assert hemm_rows(npeers=2, peer=None) == -1
+    assert hemm_rows(npeers=16, peer=peers) == -1
+    assert hemm_rows(y=X) == -1                           # in-place product is not defined
+    assert hemm_rows(alpha=float("nan")) == -1
+    assert hemm_rows(ncols=0) == 0
+    assert hemm_rows(dtype=1, N=64, nrows=24) == -6       # f64: 16-row groups
+
+    deg = np.asarray([2, 2, 4, 4], dtype=np.int32)
+    seq = C.c_uint32(0)
+
+    def rows_ws(nranks=1, rank=0, peer_v=None, peer_w=None, flags=None, peer_flags=None, a=-1.0, ws_bytes=1 << 20,
+                degrees=deg):
+        return lib.chase_filter_rows_ws(H, 64, 0, 32, X, 4, degrees.ctypes.data, a, 2.0, -2.0, 3, Y, ws_bytes,
+                                        nranks, rank, peer_v, peer_w, flags, peer_flags, C.addressof(seq), None)
+
+    assert rows_ws(nranks=0) == -1
+    assert rows_ws(nranks=2, rank=2) == -1
+    assert rows_ws(nranks=2, rank=0) == -1                # peers missing
+    assert rows_ws(flags=0x6000, peer_flags=None) == -1
+    assert rows_ws(a=3.0) == -2
+    assert rows_ws(degrees=np.asarray([4, 2, 4, 4], dtype=np.int32)) == -3
+    assert rows_ws(ws_bytes=16) == -5
+    assert seq.value == 0                                 # no barrier was enqueued
+
+    assert lib.chase_rows_barrier(None, peers, 2, 0, 1, None) == -1
+    assert lib.chase_rows_barrier(0x6000, peers, 2, 5, 1, None) == -1
+    assert lib.chase_rows_barrier(0x6000, peers, 17, 0, 1, None) == -1
+
+    al = np.zeros(10)
+    def lanczos(N=64, nruns=2, k=5, dtype=3, ws=0x7000, ws_bytes=1 << 24, v0=X):
+        return lib.chase_lanczos(H, N, v0, nruns, k, dtype, al.ctypes.data, al.ctypes.data, ws, ws_bytes, None)
+    assert lanczos(dtype=8) == -4
+    assert lanczos(k=0) == -1
+    assert lanczos(k=65) == -1                            # more steps than the dimension
+    assert lanczos(nruns=0) == -1
+    assert lanczos(v0=None) == -1
+    assert lanczos(ws=None) == -5
+    assert lanczos(ws_bytes=1024) == -5
+    assert lanczos(ws=0x7008) == -6
+    assert pkg.chase_filter_launch_count() == before
