@@ -46,8 +46,8 @@ TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one full-width step launch (ncu --set full captures).
 NCU_TRAFFIC = {
-    4: (155.942670e9 + 1.323090e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); "
-                                   "profiles/ncu_r1b_step_dmma_c128.md"),
+    4: (199.664869e9 + 1.309856e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); "
+                                   "profiles/ncu_r1d_step_dmma.md"),
     5: (129.506315e9 + 1.473567e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
                                    "profiles/ncu_r1c_step_tf32_c64.md"),
 }
