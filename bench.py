@@ -11,7 +11,10 @@ Prints ONE JSON line (rank 0).  `value` = filter GFLOP/s = 8 N^2 sum(deg) / t (c
 sum(deg) real), whole job, inputs resident in HBM.  `e2e` = same metric through
 chase_filter_host (HOST buffers, H2D/D2H inside the timed region).  `roofline` = achieved
 TFLOP/s of the step kernel vs the FP64 peak.  `cpu_baseline` = the oracle,
-as it stands, on the host cores on a bounded sample.  --impl reference times the oracle.
+as it stands, on the host cores on a bounded sample.  `parity` = the timed run's result against the
+oracle on the SURVEY 8(c) column sample (>= 32 columns, own degrees, full H).  `all_configs` = the other
+BASELINE.json configs (1, 2, 3, 5), each timed the same way with its own clock record, roofline
+fraction and oracle comparison.  --impl reference times the oracle.
 Multi-GPU (--gpus N under torchrun): independent column batches per rank, H replicated, no
 data-path collective; scaling = weak.
 """
@@ -45,11 +48,12 @@ TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one full-width step launch (ncu --set full captures).
+# NOT measured in this run: typed in from the committed capture named in each note.
 NCU_TRAFFIC = {
-    4: (199.664869e9 + 1.309856e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); "
-                                   "profiles/ncu_r1d_step_dmma.md"),
+    4: (199.664869e9 + 1.309856e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); from "
+                                   "profiles/ncu_r1d_step_dmma.md, not measured in this run"),
     5: (129.506315e9 + 1.473567e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
-                                   "profiles/ncu_r1c_step_tf32_c64.md"),
+                                   "from profiles/ncu_r1c_step_tf32_c64.md, not measured in this run"),
 }
 
 
@@ -76,6 +80,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-aux", action="store_true", help="skip the hemm / residuals / Lanczos timings")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the cfg 1/2/3/5 block of the JSON line")
     ap.add_argument("--sample-cols", type=int, default=16)
     ap.add_argument("--sample-degree", type=int, default=8)
     return ap.parse_args()
@@ -305,21 +310,18 @@ def run_reference(args):
 # ----------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------
-def run_ours(args):
-    import paper_1805_10121_b200 as pkg
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    pkg.load()
-    rank, world, local = dist_setup(args.gpus)
-    device = torch.device("cuda", local)
-    torch.cuda.set_device(device)
+DTYPE_LABEL = {torch.complex128: "c128 (f64 arithmetic)", torch.float64: "f64",
+               torch.complex64: "c64 (f32 arithmetic)", torch.float32: "f32"}
 
-    w = build_workload(args, device, rank)
+
+def time_filter(pkg, w, steps: int, warmup: int, device, world: int, rank: int, local: int):
+    """W untimed + K timed chase_filter_ws calls on workload `w` (V restored from V0 and, for inputs
+    that fit in L2, the L2 flushed outside the timed region; CUDA events on the launching stream;
+    nvidia-smi clocks sampled during the timed region).  Returns a dict; `dev_s` is this rank's."""
     N, n, dtype = w.N, w.ncols, w.dtype
     V = W.empty_colmajor(N, n, dtype, device)
     ws = torch.empty(pkg.chase_filter_workspace_bytes(N, n, dtype), dtype=torch.uint8, device=device)
     stream = torch.cuda.Stream(device)
-    flops_step = w.flops()
     h_bytes = w.H.numel() * w.H.element_size()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=device) if h_bytes < (512 << 20) else None
 
@@ -337,33 +339,29 @@ def run_ours(args):
         torch.cuda.current_stream().wait_stream(stream)
         return (e0, e1) if timed else None
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         one_step(False)
     barrier(world)
-
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
     launches0 = pkg.chase_filter_launch_count()
     barrier(world)
     t_wall0 = time.perf_counter()
-    events = [one_step(True) for _ in range(args.steps)]
+    events = [one_step(True) for _ in range(steps)]
     barrier(world)
     t_wall = time.perf_counter() - t_wall0
     launches = pkg.chase_filter_launch_count() - launches0
     clocks = sampler.stop() if rank == 0 else None
+    ms = [e0.elapsed_time(e1) for e0, e1 in events]
+    return {"dev_s": sum(ms) * 1e-3, "ms": ms, "launches": launches, "clocks": clocks, "t_wall": t_wall, "V": V}
 
-    dev_s = sum(e0.elapsed_time(e1) for e0, e1 in events) * 1e-3     # device time of the K filter calls
-    dev_s = max_over_ranks(dev_s, world)
-    total_flops = sum_over_ranks(flops_step * args.steps, world)
-    value = total_flops / dev_s * 1e-9
 
-    # ---- roofline of the step kernel (all launches of a step are the same kernel) --------------
+def roofline_of(pkg, w, achieved_tflops: float, clocks, device, launches_per_step: int, cfg_id, reduced: bool):
+    """Roofline record of the step kernel that serves workload `w`."""
+    N, n, dtype = w.N, w.ncols, w.dtype
     sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
     sms = torch.cuda.get_device_properties(device).multi_processor_count
-    probe_dmma = pkg.chase_fp64_peak_probe(1, 1 << 16) * 1e-3
-    probe_dfma = pkg.chase_fp64_peak_probe(0, 1 << 16) * 1e-3
-    achieved = flops_step * args.steps / (sum(e0.elapsed_time(e1) for e0, e1 in events) * 1e-3) * 1e-12
     kernel_path = pkg.chase_filter_kernel_path(N, n, dtype)
     is_f64 = dtype in (torch.complex128, torch.float64)
     if kernel_path == 2:
@@ -384,36 +382,139 @@ def run_ours(args):
     # DRAM bytes (read + write) of ONE full-width launch from the committed `ncu --set full` capture
     # (profiles/); only known for the two captured workloads.
     traffic, traffic_note = None, None
-    if args.N is None and args.ncols is None and args.config in NCU_TRAFFIC:
-        traffic, traffic_note = NCU_TRAFFIC[args.config]
-    roofline = {
+    if not reduced and cfg_id in NCU_TRAFFIC:
+        traffic, traffic_note = NCU_TRAFFIC[cfg_id]
+    return {
         "bound": bound, "kernel": kname,
-        "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tflops / peak,
         "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_source,
-        "peak_probe_dmma_tflops": probe_dmma, "peak_probe_dfma_tflops": probe_dfma,
-        "frac_of_probe_dmma": achieved / probe_dmma if is_f64 else None,
-        "frac_of_nvidia_quoted_40tf": achieved / 40.0 if is_f64 else None,
-        "algorithmic_flops_per_step": flops_step, "launches_per_step": launches // max(args.steps, 1),
+        "frac_of_nvidia_quoted_40tf": achieved_tflops / 40.0 if is_f64 else None,
+        "algorithmic_flops_per_step": w.flops(), "launches_per_step": launches_per_step,
     }
 
-    # ---- sampled parity + cpu_baseline (rank 0, N = 1): the oracle on a bounded sample ---------
-    cpu_baseline, parity = None, None
+
+def parity_vs_oracle(pkg, w, V_full, device, max_full_flops: float = 1.5e12):
+    """GPU result of the FULL run (V_full, every column filtered with its own degree inside the timed
+    launch configuration) against the oracle: the whole block when the oracle finishes in seconds,
+    else the SURVEY 8(c) column sample (>= 32 columns, each with its own degree, full H; pin P7)."""
+    import oracle
+    N, n = w.N, w.ncols
+    Hn = host_colmajor_numpy(w.H)
+    if w.flops() <= max_full_flops:
+        cols = list(range(n))
+        sample = f"all {n} columns, full {N}x{N} H, own degrees"
+    else:
+        cols = W.parity_sample_columns(w.degrees)
+        sample = (f"sampled: {len(cols)} of {n} columns (first/last of every degree class, tile edges, seeded random), "
+                  f"full {N}x{N} H, own degrees")
+    deg = w.degrees.numpy()[cols]
+    Vs = host_colmajor_numpy(W.as_colmajor(w.V0[:, cols]))
+    t0 = time.perf_counter()
+    ref = oracle.chase_filter(Hn, Vs, deg, w.a, w.b, w.lambda1)
+    dt = time.perf_counter() - t0
+    del Hn
+    got = host_colmajor_numpy(W.as_colmajor(V_full[:, cols]))
+    col_err = np.linalg.norm(got - ref, axis=0) / np.linalg.norm(ref, axis=0)
+    tol = 1e-12 if w.dtype in (torch.complex128, torch.float64) else 1e-4
+    rel = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+    return {"rel_fro_vs_oracle": rel, "worst_column_rel_err": float(col_err.max()), "tolerance": tol,
+            "ok": bool(rel <= tol), "sample": sample, "degrees_sampled": sorted(set(int(d) for d in deg)),
+            "oracle_seconds": dt}
+
+
+def cpu_blas_context(w, ncols: int = 128):
+    """Context only: ONE step (H - cI) X through numpy's BLAS GEMM on the host cores, on a
+    column block wide enough to be compute-bound -- what the paper's CPU path (ZHEMM, Listing 2) would
+    achieve here.  Not the oracle, not the reference arm; labelled as such."""
+    Hn = host_colmajor_numpy(w.H)
+    X = np.asfortranarray(host_colmajor_numpy(W.as_colmajor(w.V0[:, :min(ncols, w.ncols)])))
+    f = 8.0 if np.iscomplexobj(Hn) else 2.0
+    t0 = time.perf_counter()
+    Y = Hn @ X
+    Y -= 0.5 * (w.a + w.b) * X
+    dt = time.perf_counter() - t0
+    return {"what": "numpy (vendor BLAS) GEMM, one step (H - cI) X, context only", "ncols": X.shape[1],
+            "seconds": dt, "gflops": f * float(w.N) ** 2 * X.shape[1] / dt * 1e-9}
+
+
+ALL_CONFIG_STEPS = {1: 20, 2: 10, 3: 5, 5: 3}     # timed filter calls per non-headline config (3 warm-ups each)
+
+
+def run_other_configs(pkg, device, headline_cfg: int):
+    """The other BASELINE.json configs, each timed the same way as the headline one (own clock record)
+    and compared with the oracle at full size: driver-observed numbers for cfgs 1, 2, 3, 5."""
+    out = {}
+    for cfg, steps in ALL_CONFIG_STEPS.items():
+        if cfg == headline_cfg:
+            continue
+        try:
+            w = W.make_config(cfg, device=device)
+            r = time_filter(pkg, w, steps, 3, device, 1, 0, device.index or 0)
+            value = w.flops() * steps / r["dev_s"] * 1e-9
+            roof = roofline_of(pkg, w, value * 1e-3, r["clocks"], device, r["launches"] // steps, cfg, False)
+            par = parity_vs_oracle(pkg, w, r["V"], device)
+            out[f"cfg{cfg}"] = {
+                "workload": f"N={w.N} {W.DTYPE_NAMES[w.dtype]}, V0 {w.N}x{w.ncols}, degrees "
+                            f"{int(w.degrees.min())}..{int(w.degrees.max())}, sum_deg={w.sum_deg}",
+                "value": value, "unit": UNIT, "steps": steps, "warmup": 3,
+                "ms_per_step": r["dev_s"] / steps * 1e3, "ms_min": min(r["ms"]), "dtype": DTYPE_LABEL[w.dtype],
+                "roofline": roof, "clocks": r["clocks"], "gpu_launches": r["launches"],
+                "rel_fro_vs_oracle": par["rel_fro_vs_oracle"], "parity": par,
+            }
+            del r, w
+        except Exception as exc:                       # one config failing must not lose the headline line
+            out[f"cfg{cfg}"] = {"error": f"{type(exc).__name__}: {str(exc)[:300]}"}
+        torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import paper_1805_10121_b200 as pkg
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    pkg.load()
+    rank, world, local = dist_setup(args.gpus)
+    device = torch.device("cuda", local)
+    torch.cuda.set_device(device)
+
+    w = build_workload(args, device, rank)
+    N, n, dtype = w.N, w.ncols, w.dtype
+    flops_step = w.flops()
+    r = time_filter(pkg, w, args.steps, args.warmup, device, world, rank, local)
+    V, launches, clocks, t_wall = r["V"], r["launches"], r["clocks"], r["t_wall"]
+    dev_s = max_over_ranks(r["dev_s"], world)
+    total_flops = sum_over_ranks(flops_step * args.steps, world)
+    value = total_flops / dev_s * 1e-9
+
+    # ---- roofline of the step kernel (all launches of a step are the same kernel) --------------
+    is_f64 = dtype in (torch.complex128, torch.float64)
+    achieved = flops_step * args.steps / r["dev_s"] * 1e-12
+    reduced = args.N is not None or args.ncols is not None
+    roofline = roofline_of(pkg, w, achieved, clocks, device, launches // max(args.steps, 1), args.config, reduced)
+    probe_dmma = pkg.chase_fp64_peak_probe(1, 1 << 16) * 1e-3
+    probe_dfma = pkg.chase_fp64_peak_probe(0, 1 << 16) * 1e-3
+    roofline.update({"peak_probe_dmma_tflops": probe_dmma, "peak_probe_dfma_tflops": probe_dfma,
+                     "frac_of_probe_dmma": achieved / probe_dmma if is_f64 else None})
+
+    # ---- parity of the timed configuration (rank 0, N = 1): the last timed run's V vs the oracle ----
+    # ---- cpu_baseline: the oracle, as it stands, on a BOUNDED sample (about 10-30 s of CPU work) ----
+    cpu_baseline, parity, blas_ctx = None, None, None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
+        parity = parity_vs_oracle(pkg, w, V, device)
         cols = sample_columns(w, args.sample_cols)
         Hn = host_colmajor_numpy(w.H)
         Vs = W.as_colmajor(w.V0[:, cols])
-        dt, fl, ref = oracle_sample_run(Hn, host_colmajor_numpy(Vs), args.sample_degree, w)
+        dt, fl, _ = oracle_sample_run(Hn, host_colmajor_numpy(Vs), args.sample_degree, w)
         del Hn
-        wss = torch.empty(pkg.chase_filter_workspace_bytes(N, len(cols), dtype), dtype=torch.uint8, device=device)
-        pkg.chase_filter_ws(w.H, Vs, [args.sample_degree] * len(cols), w.a, w.b, w.lambda1, wss)
-        torch.cuda.synchronize()
-        got = host_colmajor_numpy(Vs)
         sample = (f"{len(cols)} of {n} columns (evenly spaced), full {N}x{N} H, degree truncated to "
                   f"{args.sample_degree}")
         cpu_baseline = {"value": fl / dt * 1e-9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                         "sample": sample, "seconds": dt}
-        parity = {"rel_fro_vs_oracle": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)), "sample": sample}
+        try:
+            blas_ctx = cpu_blas_context(w)
+        except Exception as exc:
+            blas_ctx = {"error": str(exc)[:200]}
 
     # ---- aux: the other entry points on the same workload (SURVEY 8(f)-2, -4), device-timed --------------
     aux = None
@@ -460,16 +561,27 @@ def run_ours(args):
                "api": "chase_filter_host (pinned host H, V; cudaMalloc + H2D + filter + D2H + free inside)"}
         del Hh, Vh
 
+    # ---- the other BASELINE.json configs, driver-observed (rank 0, N = 1, default workload only) --------
+    all_configs = None
+    if rank == 0 and world == 1 and not args.no_all_configs and not reduced:
+        cfg_line = workload_config(args, w, world)
+        del V, r
+        w.H = None
+        w.V0 = None
+        torch.cuda.empty_cache()
+        all_configs = run_other_configs(pkg, device, args.config)
+    else:
+        cfg_line = workload_config(args, w, world)
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dev_s / args.steps * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": {torch.complex128: "c128 (f64 arithmetic)",
-                                                               torch.float64: "f64", torch.complex64: "c64 (f32 arithmetic)",
-                                                               torch.float32: "f32"}[dtype],
-            "data": "synthetic", "config": workload_config(args, w, world), "clocks": clocks,
+            "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_LABEL[dtype],
+            "data": "synthetic", "config": cfg_line, "clocks": clocks,
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
-            "parity": parity, "aux_ops": aux, "comparator_cublas": comparator, "wall_s_timed_region": t_wall,
+            "parity": parity, "aux_ops": aux, "comparator_cublas": comparator, "cpu_blas_context": blas_ctx,
+            "all_configs": all_configs, "wall_s_timed_region": t_wall,
             "fraction_of_fp64_peak": roofline["frac"] if is_f64 else None,
         }
         print(json.dumps(line))

@@ -48,6 +48,7 @@ extern "C" {
 #endif
 
 #define CHASE_MAX_RANKS 16   /* most GPUs one row-sharded filter spans (chase_filter_rows_*) */
+#define CHASE_MAX_DEGREE 4096 /* largest accepted degrees[j]; the paper's degrees are <= 36 (Table 1) */
 
 typedef enum {
     CHASE_F32 = 0,  /* float,                 tcgen05 3xTF32 tensor path when N % 4 == 0, else FP32 FMA */
@@ -60,10 +61,12 @@ enum {
     CHASE_OK = 0,
     CHASE_ERR_ARG = -1,       /* null pointer, N <= 0, ncols < 0, N or ncols too large */
     CHASE_ERR_BOUNDS = -2,    /* not (lambda1 < a < b), or a non-finite bound (reading G8) */
-    CHASE_ERR_DEGREES = -3,   /* a negative degree, or degrees not non-decreasing (G7) */
+    CHASE_ERR_DEGREES = -3,   /* a negative degree, one above CHASE_MAX_DEGREE, or degrees not non-decreasing (G7) */
     CHASE_ERR_DTYPE = -4,     /* unknown chase_dtype_t */
     CHASE_ERR_WORKSPACE = -5, /* workspace null or smaller than chase_filter_workspace_bytes */
-    CHASE_ERR_ALIGN = -6      /* H, V or workspace not aligned to 16 bytes */
+    CHASE_ERR_ALIGN = -6,     /* H, V or workspace not aligned to 16 bytes */
+    CHASE_ERR_TIMEOUT = -7    /* row-sharded path: a peer rank did not reach an inter-GPU barrier in time
+                                 (chase_rows_status), or the caller's host barrier reported a failure */
 };
 
 /* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype` (the W of
@@ -138,7 +141,9 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
  *   Listing 1 Resd).  One step kernel with a per-column shift in the epilogue
  *   (R = H V - V diag(ritzv) into the workspace) plus one column-norm kernel.  V DEVICE (read
  *   only), ritzv HOST double[ncols] (consumed before return), resid DEVICE double[ncols],
- *   workspace DEVICE >= chase_residuals_workspace_bytes(...).  Asynchronous on `stream`. */
+ *   workspace DEVICE >= chase_residuals_workspace_bytes(...).  Asynchronous on `stream`: ritzv is copied
+ *   with one cudaMemcpyAsync, i.e. a PAGEABLE ritzv is consumed before return, a PINNED one must stay
+ *   unchanged until `stream` has drained. */
 int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
                double alpha, double beta, double shift, chase_dtype_t dtype, void *stream);
 size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
@@ -190,28 +195,53 @@ int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, cons
  *   Asynchronous; no inter-GPU synchronisation (see chase_rows_barrier).
  *
  * chase_rows_barrier: all ranks' work enqueued so far on their streams has completed, including its
- *   peer stores.  flags: this rank's DEVICE uint32[nranks], zeroed once by the caller; peer_flags: HOST
+ *   peer stores.  flags: this rank's DEVICE uint32[nranks + 1], zeroed once by the caller -- entries
+ *   [0, nranks) are the arrival slots, entry [nranks] is a STICKY status word; peer_flags: HOST
  *   array [nranks] of pointers valid on this device to every rank's flags array (entry [rank] = flags);
- *   seq: value strictly larger than any used before on these flags (same on all ranks).  Enqueues a
- *   signal kernel (system-scope release stores of seq into flags[rank] of every rank) and a wait
- *   kernel (spins, bounded to ~30 s, until all nranks entries of the local flags reach seq).
+ *   seq: value strictly larger than any used before on these flags (same on all ranks).
+ *   = chase_rows_signal (a kernel that release-stores seq, system scope, into flags[rank] of every rank)
+ *   followed by chase_rows_wait (a kernel that polls the local slots until all nranks reach seq).
+ *   The wait is bounded (30 s; environment CHASE_ROWS_TIMEOUT_MS overrides, read per call).  On a timeout
+ *   it stores the failing seq into the status word and returns, and every later wait returns at once:
+ *   the stream drains, the data are WRONG, and chase_rows_status says so.
+ *
+ * chase_rows_status: SYNCHRONISES `stream` and returns CHASE_ERR_TIMEOUT if any barrier enqueued on these
+ *   flags timed out since they were zeroed, else 0.  Call it before using the result of a row-sharded
+ *   filter.
  *
  * chase_filter_rows_ws: the filter of chase_filter_ws on a row-sharded H: per degree step one
  *   chase_hemm_rows launch on the active suffix and one chase_rows_barrier.  V (in: V_0 complete on
  *   every rank; out: result complete on every rank) and workspace as in chase_filter_ws; peer_V /
  *   peer_W: HOST arrays [nranks] of peer-mapped pointers to every rank's V / workspace (entry [rank]
  *   ignored); *seq (HOST, in/out) carries the barrier sequence across calls (start at 0).
- *   flags == NULL skips the barriers (single rank, or a caller that serialises the ranks itself). */
+ *   flags == NULL skips the barriers (single rank, or a caller that serialises the ranks itself).
+ *
+ * chase_filter_rows_hostsync_ws: same, for ranks that TIME-SHARE one GPU (several processes per device:
+ *   their kernels are not guaranteed to run concurrently, so a spinning wait kernel could keep the peer's
+ *   kernels off the GPU).  Every barrier becomes: signal kernel, cudaStreamSynchronize, host_barrier(ctx)
+ *   (the caller's inter-process barrier, e.g. over gloo / MPI; non-zero return = failure ->
+ *   CHASE_ERR_TIMEOUT), then the wait kernel, which finds every flag already set.  host_barrier == NULL is
+ *   chase_filter_rows_ws.  Synchronises; not capturable. */
 int chase_hemm_rows(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, const void *X, void *Y,
                     int64_t ncols, double alpha, double beta, double shift, chase_dtype_t dtype,
                     int32_t npeers, void *const *peer_Y, void *stream);
 int chase_rows_barrier(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank,
                        uint32_t seq, void *stream);
+int chase_rows_signal(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank,
+                      uint32_t seq, void *stream);
+int chase_rows_wait(uint32_t *flags, int32_t nranks, uint32_t seq, void *stream);
+int chase_rows_status(const uint32_t *flags, int32_t nranks, void *stream);
 int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
                          const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
                          void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
                          void *const *peer_V, void *const *peer_W, uint32_t *flags,
                          uint32_t *const *peer_flags, uint32_t *seq, void *stream);
+int chase_filter_rows_hostsync_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
+                                  const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
+                                  void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
+                                  void *const *peer_V, void *const *peer_W, uint32_t *flags,
+                                  uint32_t *const *peer_flags, uint32_t *seq, void *stream,
+                                  int (*host_barrier)(void *), void *host_ctx);
 
 /* CUDA IPC plumbing for the peer pointers above (one process per GPU).  chase_ipc_export: handle
  * (HOST, 64 bytes) of the allocation containing dev_ptr and dev_ptr's byte offset inside it.

@@ -23,9 +23,11 @@ EXPORTS = [
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
     "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_tiling",
     "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates",
-    "chase_hemm_rows", "chase_rows_barrier", "chase_filter_rows_ws", "chase_ipc_export", "chase_ipc_open",
+    "chase_hemm_rows", "chase_rows_barrier", "chase_rows_signal", "chase_rows_wait", "chase_rows_status",
+    "chase_filter_rows_ws", "chase_filter_rows_hostsync_ws", "chase_ipc_export", "chase_ipc_open",
     "chase_ipc_close",
 ]
+HOST_BARRIER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
 
 _lib = None
 
@@ -91,9 +93,17 @@ def load() -> ctypes.CDLL:
     lib.chase_hemm_rows.argtypes = [vp, i64, i64, i64, vp, vp, i64, dbl, dbl, dbl, ctypes.c_int, i32, vp, vp]
     lib.chase_rows_barrier.restype = ctypes.c_int
     lib.chase_rows_barrier.argtypes = [vp, vp, i32, i32, ctypes.c_uint32, vp]
+    lib.chase_rows_signal.restype = ctypes.c_int
+    lib.chase_rows_signal.argtypes = [vp, vp, i32, i32, ctypes.c_uint32, vp]
+    lib.chase_rows_wait.restype = ctypes.c_int
+    lib.chase_rows_wait.argtypes = [vp, i32, ctypes.c_uint32, vp]
+    lib.chase_rows_status.restype = ctypes.c_int
+    lib.chase_rows_status.argtypes = [vp, i32, vp]
     lib.chase_filter_rows_ws.restype = ctypes.c_int
     lib.chase_filter_rows_ws.argtypes = [vp, i64, i64, i64, vp, i64, vp, dbl, dbl, dbl, ctypes.c_int, vp, sz,
                                          i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.chase_filter_rows_hostsync_ws.restype = ctypes.c_int
+    lib.chase_filter_rows_hostsync_ws.argtypes = lib.chase_filter_rows_ws.argtypes + [HOST_BARRIER_FN, vp]
     lib.chase_ipc_export.restype = ctypes.c_int
     lib.chase_ipc_export.argtypes = [vp, vp, vp]
     lib.chase_ipc_open.restype = ctypes.c_int
@@ -392,24 +402,51 @@ def chase_hemm_rows(H_loc: torch.Tensor, row0: int, X: torch.Tensor, Y: torch.Te
     return Y
 
 
+def _check_flags(flags: torch.Tensor, nranks: int) -> None:
+    if not flags.is_cuda or flags.dtype != torch.int32 or flags.numel() < nranks + 1:
+        raise ValueError("flags must be a CUDA int32 tensor with nranks + 1 entries (slots + status word)")
+
+
 def chase_rows_barrier(flags: torch.Tensor, peer_flags: Sequence[int], rank: int, seq: int,
                        stream: Optional[torch.cuda.Stream] = None) -> None:
     """Inter-GPU barrier on `stream` over flag arrays in peer memory (see include/chase_filter.h)."""
-    if not flags.is_cuda or flags.dtype != torch.int32 or flags.numel() < len(peer_flags):
-        raise ValueError("flags must be a CUDA int32 tensor with one entry per rank")
+    _check_flags(flags, len(peer_flags))
     arr = _ptr_array(peer_flags)
     with torch.cuda.device(flags.device):
         _check(load().chase_rows_barrier(flags.data_ptr(), arr, len(peer_flags), int(rank), int(seq) & 0xFFFFFFFF,
                                          _stream_ptr(stream)))
 
 
+def chase_rows_signal(flags: torch.Tensor, peer_flags: Sequence[int], rank: int, seq: int,
+                      stream: Optional[torch.cuda.Stream] = None) -> None:
+    _check_flags(flags, len(peer_flags))
+    arr = _ptr_array(peer_flags)
+    with torch.cuda.device(flags.device):
+        _check(load().chase_rows_signal(flags.data_ptr(), arr, len(peer_flags), int(rank), int(seq) & 0xFFFFFFFF,
+                                        _stream_ptr(stream)))
+
+
+def chase_rows_wait(flags: torch.Tensor, nranks: int, seq: int, stream: Optional[torch.cuda.Stream] = None) -> None:
+    _check_flags(flags, nranks)
+    with torch.cuda.device(flags.device):
+        _check(load().chase_rows_wait(flags.data_ptr(), int(nranks), int(seq) & 0xFFFFFFFF, _stream_ptr(stream)))
+
+
+def chase_rows_status(flags: torch.Tensor, nranks: int, stream: Optional[torch.cuda.Stream] = None) -> None:
+    """Synchronises `stream`; raises ChaseFilterError(-7) if a barrier on these flags timed out."""
+    _check_flags(flags, nranks)
+    with torch.cuda.device(flags.device):
+        _check(load().chase_rows_status(flags.data_ptr(), int(nranks), _stream_ptr(stream)))
+
+
 def chase_filter_rows_ws(H_loc: torch.Tensor, row0: int, V: torch.Tensor, degrees, a: float, b: float,
                          lambda1: float, workspace: torch.Tensor, rank: int = 0, peer_V: Sequence[int] = (),
                          peer_W: Sequence[int] = (), flags: Optional[torch.Tensor] = None,
                          peer_flags: Sequence[int] = (), seq: int = 0,
-                         stream: Optional[torch.cuda.Stream] = None) -> int:
+                         stream: Optional[torch.cuda.Stream] = None, host_barrier=None) -> int:
     """Row-sharded filter; peer_V / peer_W / peer_flags hold one device pointer per rank (own entry
-    ignored).  Returns the advanced barrier sequence number."""
+    ignored).  `host_barrier` (a callable returning 0) selects chase_filter_rows_hostsync_ws, for ranks
+    that time-share one GPU.  Returns the advanced barrier sequence number."""
     N, ncols = V.shape
     nrows = _check_rows(H_loc, N, row0)
     if not V.is_cuda or V.dtype != H_loc.dtype:
@@ -417,15 +454,21 @@ def chase_filter_rows_ws(H_loc: torch.Tensor, row0: int, V: torch.Tensor, degree
     _check_colmajor(V, "V")
     deg = _degrees_array(degrees, ncols)
     nranks = max(len(peer_V), 1)
+    if flags is not None:
+        _check_flags(flags, nranks)
     seq_c = ctypes.c_uint32(int(seq) & 0xFFFFFFFF)
-    with torch.cuda.device(H_loc.device):
-        _check(load().chase_filter_rows_ws(
-            H_loc.data_ptr(), N, int(row0), nrows, V.data_ptr(), ncols, deg.ctypes.data, float(a), float(b),
+    args = [H_loc.data_ptr(), N, int(row0), nrows, V.data_ptr(), ncols, deg.ctypes.data, float(a), float(b),
             float(lambda1), _DTYPE_CODE[H_loc.dtype], workspace.data_ptr(),
             workspace.numel() * workspace.element_size(), nranks, int(rank),
             _ptr_array(peer_V) if len(peer_V) else None, _ptr_array(peer_W) if len(peer_W) else None,
             flags.data_ptr() if flags is not None else None,
-            _ptr_array(peer_flags) if len(peer_flags) else None, ctypes.addressof(seq_c), _stream_ptr(stream)))
+            _ptr_array(peer_flags) if len(peer_flags) else None, ctypes.addressof(seq_c), _stream_ptr(stream)]
+    with torch.cuda.device(H_loc.device):
+        if host_barrier is None:
+            _check(load().chase_filter_rows_ws(*args))
+        else:
+            cb = HOST_BARRIER_FN(lambda _ctx: int(host_barrier() or 0))
+            _check(load().chase_filter_rows_hostsync_ws(*args, cb, None))
     return int(seq_c.value)
 
 

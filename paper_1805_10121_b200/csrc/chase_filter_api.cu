@@ -5,6 +5,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstdlib>
+#include <exception>
 #include <vector>
 
 #include "chase_internal.h"
@@ -34,10 +35,11 @@ const char *chase_filter_strerror(int code) {
         case CHASE_OK: return "success";
         case CHASE_ERR_ARG: return "invalid argument (null pointer or bad size)";
         case CHASE_ERR_BOUNDS: return "bounds must satisfy lambda1 < a < b and be finite";
-        case CHASE_ERR_DEGREES: return "degrees must be >= 0 and non-decreasing";
+        case CHASE_ERR_DEGREES: return "degrees must be >= 0, <= CHASE_MAX_DEGREE and non-decreasing";
         case CHASE_ERR_DTYPE: return "unknown dtype";
         case CHASE_ERR_WORKSPACE: return "workspace missing or too small";
         case CHASE_ERR_ALIGN: return "H, V and workspace must be 16-byte aligned";
+        case CHASE_ERR_TIMEOUT: return "a peer rank did not reach an inter-GPU barrier in time";
         default:
             if (code > 0) return cudaGetErrorString((cudaError_t)code);
             return "unknown error";
@@ -81,7 +83,7 @@ int chase_filter_schedule(const int32_t *degrees, int64_t ncols, int32_t *offset
     if (ncols < 0 || ncols > kMaxDim || (ncols > 0 && !degrees)) return CHASE_ERR_ARG;
     int32_t prev = 0;
     for (int64_t j = 0; j < ncols; ++j) {
-        if (degrees[j] < 0 || degrees[j] < prev) return CHASE_ERR_DEGREES;
+        if (degrees[j] < 0 || degrees[j] < prev || degrees[j] > CHASE_MAX_DEGREE) return CHASE_ERR_DEGREES;
         prev = degrees[j];
     }
     const int32_t m_max = ncols ? degrees[ncols - 1] : 0;
@@ -103,6 +105,7 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
     if (ncols > 0 && (!resid || !ritzv || !degrees_out)) return CHASE_ERR_ARG;
     if (!(std::isfinite(a) && std::isfinite(b)) || !(a < b)) return CHASE_ERR_BOUNDS;
     const double c = 0.5 * (b + a), e = 0.5 * (b - a);
+    try {                                   // no C++ exception may cross the C ABI
     std::vector<int32_t> deg((size_t)ncols);
     for (int64_t j = 0; j < ncols; ++j) {
         if (!(resid[j] > 0.0) || !std::isfinite(resid[j]) || !std::isfinite(ritzv[j])) return CHASE_ERR_ARG;
@@ -126,6 +129,9 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
     for (int64_t i = 0; i < ncols; ++i) {
         degrees_out[i] = deg[(size_t)order[(size_t)i]];
         if (perm_out) perm_out[i] = order[(size_t)i];
+    }
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
     }
     return CHASE_OK;
 }
@@ -204,10 +210,9 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
     if (((uintptr_t)H | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
     const size_t r_bytes = chase_filter_workspace_bytes(N, ncols, dtype);
     double *d_shift = (double *)((char *)workspace + r_bytes);
-    // ritzv is consumed before return: stage it through a pinned-free synchronous-safe copy
+    // A pageable source is staged by the runtime before cudaMemcpyAsync returns (consumed before return);
+    // a pinned one is read in stream order (see the header): no synchronisation either way.
     cudaError_t e = cudaMemcpyAsync(d_shift, ritzv, (size_t)ncols * sizeof(double), cudaMemcpyHostToDevice, stream);
-    if (e != cudaSuccess) return (int)e;
-    e = cudaStreamSynchronize(stream);      // pageable source: make "consumed before return" true
     if (e != cudaSuccess) return (int)e;
     int rc = launch_one_step(H, N, V, workspace, ncols, 1.0, 0.0, 0.0, d_shift, 0, dtype, stream);
     if (rc != CHASE_OK) return rc;
@@ -228,7 +233,11 @@ int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nvec, int32_
     if (!H || !V0 || !alpha || !beta) return CHASE_ERR_ARG;
     if (!workspace || workspace_bytes < lanczos_workspace_bytes(N, nvec, k, w)) return CHASE_ERR_WORKSPACE;
     if (((uintptr_t)H | (uintptr_t)V0 | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
-    return (int)lanczos_run(H, N, V0, (int)nvec, k, dtype, w, workspace, alpha, beta, (cudaStream_t)stream_);
+    try {
+        return (int)lanczos_run(H, N, V0, (int)nvec, k, dtype, w, workspace, alpha, beta, (cudaStream_t)stream_);
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
+    }
 }
 
 int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, const double *beta, int64_t N,
@@ -236,6 +245,7 @@ int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, cons
     if (k <= 0 || nruns <= 0 || !alpha || !beta || !b_sup || N <= 0) return CHASE_ERR_ARG;
     for (int64_t i = 0; i < nruns * k; ++i)
         if (!std::isfinite(alpha[i]) || !std::isfinite(beta[i]) || beta[i] < 0.0) return CHASE_ERR_ARG;
+    try {
     std::vector<double> lam, wt;
     if (!lanczos_ritz(k, alpha, beta, lam, wt)) return CHASE_ERR_ARG;
     *b_sup = beta[k - 1] + *std::max_element(lam.begin(), lam.end());          // Alg. 6 l.3
@@ -270,6 +280,9 @@ int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, cons
     }
     *mu_ne = 0.5 * (lo + hi);
     *mu_1 = mu1;
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
+    }
     return CHASE_OK;
 }
 
@@ -333,11 +346,12 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
         return CHASE_ERR_WORKSPACE;
     if (((uintptr_t)H | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
 
-    std::vector<int32_t> offset(m_max + 1);
-    std::vector<double> alpha(m_max + 1), beta(m_max + 1);
+    // m_max <= CHASE_MAX_DEGREE (chase_filter_schedule): fixed-size plans, no allocation that could throw
+    int32_t offset[CHASE_MAX_DEGREE + 1];
+    double alpha[CHASE_MAX_DEGREE + 1], beta[CHASE_MAX_DEGREE + 1];
     double c = 0.0;
-    chase_filter_schedule(degrees, ncols, offset.data());
-    int rc = chase_filter_scalars(a, b, lambda1, m_max, alpha.data(), beta.data(), &c);
+    chase_filter_schedule(degrees, ncols, offset);
+    int rc = chase_filter_scalars(a, b, lambda1, m_max, alpha, beta, &c);
     if (rc != CHASE_OK) return rc;
 
     // Two buffers, roles swapped after every step (Alg. 4 l.10; Listing 2):
@@ -375,12 +389,18 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
             const int64_t tiles = (N + 127) / 128;
             const int panels = (int)std::min<int64_t>(8, tiles);
             const int64_t rows_per = (tiles + panels - 1) / panels * 128;
-            std::vector<cudaEvent_t> ev;
+            struct Events {                 // destroyed on every exit path
+                cudaEvent_t ev[8];
+                int n = 0;
+                ~Events() { for (int i = 0; i < n; ++i) cudaEventDestroy(ev[i]); }
+            } evs;
+            cudaEvent_t *ev = evs.ev;
             for (int64_t r0 = 0; r0 < N; r0 += rows_per) {
                 const int64_t rows = std::min(rows_per, N - r0);
                 cudaEvent_t evp;
+                if (evs.n >= 8) return CHASE_ERR_ARG;
                 if ((e = cudaEventCreateWithFlags(&evp, cudaEventDisableTiming)) != cudaSuccess) return (int)e;
-                ev.push_back(evp);
+                ev[evs.n++] = evp;
                 e = cudaMemcpy2DAsync((char *)const_cast<void *>(H) + (size_t)r0 * w, (size_t)N * w,
                                       (const char *)up->H_host + (size_t)r0 * w, (size_t)N * w, (size_t)rows * w,
                                       (size_t)N, cudaMemcpyHostToDevice, up->copy_stream);
@@ -395,7 +415,6 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
                 if ((e = dmma_plan_create_panel(&pp, dtype, H, N, r0, rows, V, workspace, ncols)) != cudaSuccess) return (int)e;
                 if ((e = dmma_launch_step(&pp, src, s, alpha[k], beta[k], c, 0, stream)) != cudaSuccess) return (int)e;
             }
-            for (cudaEvent_t evp : ev) cudaEventDestroy(evp);
             continue;
         }
         if (use_dmma) {

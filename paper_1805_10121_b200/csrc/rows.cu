@@ -6,6 +6,7 @@
 #include <cuda.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -26,20 +27,44 @@ __global__ void rows_signal_kernel(PeerFlags peers, int nranks, int rank, uint32
     }
 }
 
-// Wait until every slot of the local flag array has reached `seq`; gives up after ~30 s of polling
-// (a dead peer must not hang the GPU).
-__global__ void rows_wait_kernel(const uint32_t *flags, int nranks, uint32_t seq) {
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// Wait until every slot of the local flag array has reached `seq`.  A dead or slow peer must neither
+// hang the GPU nor go unnoticed: after `timeout_ns` of polling the kernel stores `seq` into the STICKY
+// status word flags[nranks] (first failure wins) and returns; once the word is set, later waits return
+// at once, so a failed exchange costs one timeout, and chase_rows_status reports it to the host.
+__global__ void rows_wait_kernel(uint32_t *flags, int nranks, uint32_t seq, unsigned long long timeout_ns) {
+    uint32_t *status = flags + nranks;
     if ((int)threadIdx.x < nranks) {
-        const long long t0 = clock64();
+        const unsigned long long t0 = global_ns();
         for (;;) {
             uint32_t v;
             asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flags + threadIdx.x) : "memory");
             if ((int)(v - seq) >= 0) break;
-            if (clock64() - t0 > 60000000000LL) break;     // ~30 s at 2 GHz
+            if (*(volatile uint32_t *)status != 0u) break;                 // an earlier barrier already failed
+            if (global_ns() - t0 > timeout_ns) {
+                atomicCAS(status, 0u, seq ? seq : 0xFFFFFFFFu);
+                break;
+            }
             __nanosleep(200);
         }
     }
     __syncthreads();
+}
+
+unsigned long long rows_timeout_ns() {
+    const char *env = std::getenv("CHASE_ROWS_TIMEOUT_MS");
+    long long ms = 30000;
+    if (env && env[0]) {
+        char *end = nullptr;
+        const long long v = std::strtoll(env, &end, 10);
+        if (end != env && v > 0) ms = v;
+    }
+    return (unsigned long long)ms * 1000000ull;
 }
 
 size_t elem_size(chase_dtype_t dtype) { return dtype == CHASE_C128 ? 16 : 8; }
@@ -86,34 +111,63 @@ int chase_hemm_rows(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, c
     return (int)dmma_launch_step(&plan, 0, 0, alpha, beta, shift, beta != 0.0, (cudaStream_t)stream_);
 }
 
-int chase_rows_barrier(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank, uint32_t seq,
-                       void *stream_) {
+static int fill_peer_flags(PeerFlags &pf, uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank) {
     if (!flags || !peer_flags || nranks < 1 || nranks > CHASE_MAX_RANKS || rank < 0 || rank >= nranks)
         return CHASE_ERR_ARG;
-    PeerFlags pf;
     for (int q = 0; q < nranks; ++q) {
         pf.p[q] = q == rank ? flags : peer_flags[q];
         if (!pf.p[q]) return CHASE_ERR_ARG;
     }
-    cudaStream_t stream = (cudaStream_t)stream_;
-    rows_signal_kernel<<<1, 32, 0, stream>>>(pf, nranks, rank, seq);
-    rows_wait_kernel<<<1, 32, 0, stream>>>(flags, nranks, seq);
-    count_launch();
+    return CHASE_OK;
+}
+
+int chase_rows_signal(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank, uint32_t seq,
+                      void *stream_) {
+    PeerFlags pf;
+    int rc = fill_peer_flags(pf, flags, peer_flags, nranks, rank);
+    if (rc != CHASE_OK) return rc;
+    rows_signal_kernel<<<1, 32, 0, (cudaStream_t)stream_>>>(pf, nranks, rank, seq);
     count_launch();
     return (int)cudaGetLastError();
 }
 
-int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
-                         const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
-                         void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
-                         void *const *peer_V, void *const *peer_W, uint32_t *flags,
-                         uint32_t *const *peer_flags, uint32_t *seq, void *stream_) {
+int chase_rows_wait(uint32_t *flags, int32_t nranks, uint32_t seq, void *stream_) {
+    if (!flags || nranks < 1 || nranks > CHASE_MAX_RANKS) return CHASE_ERR_ARG;
+    rows_wait_kernel<<<1, 32, 0, (cudaStream_t)stream_>>>(flags, nranks, seq, rows_timeout_ns());
+    count_launch();
+    return (int)cudaGetLastError();
+}
+
+int chase_rows_barrier(uint32_t *flags, uint32_t *const *peer_flags, int32_t nranks, int32_t rank, uint32_t seq,
+                       void *stream_) {
+    int rc = chase_rows_signal(flags, peer_flags, nranks, rank, seq, stream_);
+    if (rc != CHASE_OK) return rc;
+    return chase_rows_wait(flags, nranks, seq, stream_);
+}
+
+int chase_rows_status(const uint32_t *flags, int32_t nranks, void *stream_) {
+    if (!flags || nranks < 1 || nranks > CHASE_MAX_RANKS) return CHASE_ERR_ARG;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    uint32_t status = 0;
+    cudaError_t e = cudaMemcpyAsync(&status, flags + nranks, sizeof(status), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return (int)e;
+    return status == 0 ? CHASE_OK : CHASE_ERR_TIMEOUT;
+}
+
+int chase_filter_rows_hostsync_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
+                                  const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
+                                  void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
+                                  void *const *peer_V, void *const *peer_W, uint32_t *flags,
+                                  uint32_t *const *peer_flags, uint32_t *seq, void *stream_,
+                                  int (*host_barrier)(void *), void *host_ctx) {
     cudaStream_t stream = (cudaStream_t)stream_;
     int rc = check_rows_args(H_loc, N, row0, nrows, ncols, dtype);
     if (rc != CHASE_OK) return rc;
     if (nranks < 1 || nranks > CHASE_MAX_RANKS || rank < 0 || rank >= nranks) return CHASE_ERR_ARG;
     if (nranks > 1 && (!peer_V || !peer_W)) return CHASE_ERR_ARG;
     if (flags && (!peer_flags || !seq)) return CHASE_ERR_ARG;
+    if (host_barrier && !flags) return CHASE_ERR_ARG;
     if (ncols > 0 && (!V || !degrees)) return CHASE_ERR_ARG;
     if (!(std::isfinite(a) && std::isfinite(b) && std::isfinite(lambda1))) return CHASE_ERR_BOUNDS;
     if (!(lambda1 < a && a < b)) return CHASE_ERR_BOUNDS;
@@ -125,11 +179,11 @@ int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nro
     if (!workspace || workspace_bytes < vb) return CHASE_ERR_WORKSPACE;
     if (((uintptr_t)H_loc | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
 
-    std::vector<int32_t> offset(m_max + 1);
-    std::vector<double> alpha(m_max + 1), beta(m_max + 1);
+    int32_t offset[CHASE_MAX_DEGREE + 1];
+    double alpha[CHASE_MAX_DEGREE + 1], beta[CHASE_MAX_DEGREE + 1];
     double c = 0.0;
-    chase_filter_schedule(degrees, ncols, offset.data());
-    rc = chase_filter_scalars(a, b, lambda1, m_max, alpha.data(), beta.data(), &c);
+    chase_filter_schedule(degrees, ncols, offset);
+    rc = chase_filter_scalars(a, b, lambda1, m_max, alpha, beta, &c);
     if (rc != CHASE_OK) return rc;
 
     DmmaPlan plan;
@@ -143,14 +197,30 @@ int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nro
         plan.peer_buf[1][i] = peer_W[q];
         ++i;
     }
+    // One inter-GPU barrier: signal on the stream; then either the device-side wait (one GPU per rank, the
+    // ranks' kernels run concurrently) or, with a host barrier (ranks that time-share a GPU, where a
+    // spinning wait kernel would keep the peer's kernels from running): drain the stream, meet the other
+    // ranks on the host, and enqueue the wait, which then finds every flag already set.
+    auto sync_ranks = [&]() -> int {
+        if (!flags) return CHASE_OK;
+        const uint32_t s = ++*seq;
+        int r = chase_rows_signal(flags, peer_flags, nranks, rank, s, stream_);
+        if (r != CHASE_OK) return r;
+        if (host_barrier) {
+            cudaError_t es = cudaStreamSynchronize(stream);
+            if (es != cudaSuccess) return (int)es;
+            if (host_barrier(host_ctx) != 0) return CHASE_ERR_TIMEOUT;
+        }
+        return chase_rows_wait(flags, nranks, s, stream_);
+    };
     // Before step 1 overwrites the peers' scratch rows, every rank must have entered the call
     // (its previous use of the scratch buffer is over) -- and after each step k every rank must have
     // finished it: all rows of V_k have landed everywhere and nobody still reads V_{k-1}.
-    if (flags && (rc = chase_rows_barrier(flags, peer_flags, nranks, rank, ++*seq, stream_)) != CHASE_OK) return rc;
+    if ((rc = sync_ranks()) != CHASE_OK) return rc;
     for (int k = 1; k <= m_max; ++k) {
         e = dmma_launch_step(&plan, (k - 1) & 1, offset[k], alpha[k], beta[k], c, k > 1, stream);
         if (e != cudaSuccess) return (int)e;
-        if (flags && (rc = chase_rows_barrier(flags, peer_flags, nranks, rank, ++*seq, stream_)) != CHASE_OK) return rc;
+        if ((rc = sync_ranks()) != CHASE_OK) return rc;
     }
     // odd-degree columns ended in the scratch buffer, which is complete on every rank: local copy back
     const size_t col_bytes = (size_t)N * w;
@@ -164,6 +234,16 @@ int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nro
         j = j1;
     }
     return CHASE_OK;
+}
+
+int chase_filter_rows_ws(const void *H_loc, int64_t N, int64_t row0, int64_t nrows, void *V, int64_t ncols,
+                         const int32_t *degrees, double a, double b, double lambda1, chase_dtype_t dtype,
+                         void *workspace, size_t workspace_bytes, int32_t nranks, int32_t rank,
+                         void *const *peer_V, void *const *peer_W, uint32_t *flags,
+                         uint32_t *const *peer_flags, uint32_t *seq, void *stream_) {
+    return chase_filter_rows_hostsync_ws(H_loc, N, row0, nrows, V, ncols, degrees, a, b, lambda1, dtype, workspace,
+                                         workspace_bytes, nranks, rank, peer_V, peer_W, flags, peer_flags, seq,
+                                         stream_, nullptr, nullptr);
 }
 
 int chase_ipc_export(const void *dev_ptr, void *handle64, int64_t *offset) {

@@ -95,9 +95,14 @@ class RowShardedFilter:
         f = RowShardedFilter(H_loc, row0, N, ncols, rank, world)
         f.V.copy_(V0)                    # every rank fills the complete V0
         f.run(degrees, a, b, lambda1)    # f.V then holds the complete result on every rank
+
+    `host_barrier` (a callable, e.g. torch.distributed.barrier over gloo) must be given when several
+    ranks share ONE GPU: their kernels time-slice, so the inter-GPU barrier is then sequenced on the host
+    (chase_filter_rows_hostsync_ws) instead of by a spinning kernel.  run() ends with chase_rows_status:
+    a barrier that timed out raises instead of returning a half-gathered result.
     """
 
-    def __init__(self, H_loc, row0: int, N: int, ncols: int, rank: int, world: int):
+    def __init__(self, H_loc, row0: int, N: int, ncols: int, rank: int, world: int, host_barrier=None):
         import torch
         from . import binding, workloads
         self.binding = binding
@@ -105,8 +110,9 @@ class RowShardedFilter:
         dev, dtype = H_loc.device, H_loc.dtype
         self.V = workloads.empty_colmajor(N, ncols, dtype, dev)
         self.W = workloads.empty_colmajor(N, ncols, dtype, dev)
-        self.flags = torch.zeros(world, dtype=torch.int32, device=dev)
+        self.flags = torch.zeros(world + 1, dtype=torch.int32, device=dev)    # arrival slots + sticky status word
         self.seq = 0
+        self.host_barrier = host_barrier
         if world > 1:
             with torch.cuda.device(dev):
                 self.table, self._bases = exchange_peer_pointers(
@@ -120,7 +126,8 @@ class RowShardedFilter:
         self.seq = self.binding.chase_filter_rows_ws(
             self.H_loc, self.row0, self.V, degrees, a, b, lambda1, ws, rank=self.rank,
             peer_V=self.table["V"], peer_W=self.table["W"], flags=self.flags,
-            peer_flags=self.table["flags"], seq=self.seq, stream=stream)
+            peer_flags=self.table["flags"], seq=self.seq, stream=stream, host_barrier=self.host_barrier)
+        self.binding.chase_rows_status(self.flags, self.world, stream)        # raises on a timed-out barrier
         return self.V
 
     @staticmethod

@@ -252,3 +252,31 @@ def reflector_hermitian(N: int, dtype, seed: int, device="cpu", nreflect: int = 
         d = torch.arange(N, device=device)
         Hd[d, d] = Hd[d, d].real.to(wide)
     return as_colmajor(Hd.to(dtype)), lam, us
+
+
+def parity_sample_columns(degrees, min_cols: int = 32, tile_widths=(64, 128), seed: int = BASE_SEED + 7):
+    """Column sample for parity at sizes where the oracle cannot run the full block (SURVEY 8(c)
+    "Where the oracle runs in full vs sampled"): the first and last column of EVERY distinct degree
+    (i.e. both sides of every column drop of Alg. 4 l.12-14), the global first / last column, the
+    columns at -1 / 0 / +1 around the first multiples of the kernels' column-tile widths, the middle
+    column, and seeded random columns up to `min_cols`.  Returns sorted unique indices; each sampled
+    column keeps its own degree (columns are independent, pin P7)."""
+    deg = [int(d) for d in (degrees.tolist() if hasattr(degrees, "tolist") else degrees)]
+    n = len(deg)
+    if n == 0:
+        return []
+    cols = {0, n - 1, n // 2}
+    for j in range(n):
+        if j == 0 or deg[j] != deg[j - 1]:
+            cols.add(j)
+            if j > 0:
+                cols.add(j - 1)
+    for w in tile_widths:
+        for mult in (1, 2):
+            for d in (-1, 0, 1):
+                cols.add(w * mult + d)
+    cols = {c for c in cols if 0 <= c < n}
+    g = _gen(seed, "cpu")
+    while len(cols) < min(min_cols, n):
+        cols.add(int(torch.randint(0, n, (1,), generator=g).item()))
+    return sorted(cols)

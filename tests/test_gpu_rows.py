@@ -77,7 +77,7 @@ def test_filter_rows_single_rank_equals_plain_filter(with_flags):
     V1, V2 = _dev(w.V0), _dev(w.V0)
     ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=DEV)
     pkg.chase_filter_ws(H, V1, w.degrees, w.a, w.b, w.lambda1, ws)
-    flags = torch.zeros(1, dtype=torch.int32, device=DEV) if with_flags else None
+    flags = torch.zeros(2, dtype=torch.int32, device=DEV) if with_flags else None      # slot + status word
     seq = pkg.chase_filter_rows_ws(H, 0, V2, w.degrees, w.a, w.b, w.lambda1, ws, rank=0,
                                    flags=flags, peer_flags=[flags.data_ptr()] if with_flags else [], seq=5)
     torch.cuda.synchronize()
@@ -85,6 +85,8 @@ def test_filter_rows_single_rank_equals_plain_filter(with_flags):
     if with_flags:
         m_max = int(w.degrees.max())
         assert seq == 5 + 1 + m_max and int(flags.cpu()[0]) == seq      # one barrier on entry, one per step
+        pkg.chase_rows_status(flags, 1)                                 # no barrier timed out
+        assert int(flags.cpu()[1]) == 0
 
 
 def test_rows_rejects_unsupported_layouts():
@@ -111,3 +113,100 @@ def test_row_sharded_filter_class_single_rank():
     assert rel_fro(f.V.cpu().numpy(), ref) <= 1e-12
     assert f.seq == 1 + int(w.degrees.max())
     f.close()
+
+
+def test_barrier_whose_peer_never_signals_fails_loudly(monkeypatch):
+    """A dead peer must not produce CHASE_OK: the wait kernel gives up after the (overridden, short)
+    timeout, sets the sticky status word, later waits return at once, and chase_rows_status raises
+    CHASE_ERR_TIMEOUT (-7).  One kernel polls alone for 100 ms; nothing waits on another kernel."""
+    monkeypatch.setenv("CHASE_ROWS_TIMEOUT_MS", "100")
+    flags = torch.zeros(3, dtype=torch.int32, device=DEV)            # 2 ranks + status word
+    dead_peer = torch.zeros(3, dtype=torch.int32, device=DEV)        # rank 1's array; rank 1 never runs
+    peers = [flags.data_ptr(), dead_peer.data_ptr()]
+    import time
+    t0 = time.perf_counter()
+    pkg.chase_rows_barrier(flags, peers, rank=0, seq=1)
+    pkg.chase_rows_barrier(flags, peers, rank=0, seq=2)              # returns at once: status already set
+    with pytest.raises(pkg.ChaseFilterError) as e:
+        pkg.chase_rows_status(flags, 2)
+    dt = time.perf_counter() - t0
+    assert e.value.code == -7
+    assert 0.05 < dt < 5.0, dt
+    f = flags.cpu().numpy()
+    assert f[0] == 2 and f[1] == 0 and f[2] == 1                     # own slot signalled, peer silent, failed at seq 1
+    assert int(dead_peer.cpu()[0]) == 2                              # the signal did reach the peer's array
+    # a filter on these flags reports the failure too
+    w = W.make_config(2, N=520, ncols=16)
+    H, V = _dev(w.H), _dev(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=DEV)
+    other_V, other_W = _dev(w.V0), _dev(w.V0)
+    pkg.chase_filter_rows_ws(H, 0, V, w.degrees, w.a, w.b, w.lambda1, ws, rank=0,
+                             peer_V=[0, other_V.data_ptr()], peer_W=[0, other_W.data_ptr()],
+                             flags=flags, peer_flags=peers, seq=2)
+    with pytest.raises(pkg.ChaseFilterError) as e:
+        pkg.chase_rows_status(flags, 2)
+    assert e.value.code == -7
+
+
+def _two_process_worker(rank, world, port, N, n, dtype_name, q):
+    """One REAL process per rank, both on cuda:0: real chase_ipc_export / chase_ipc_open of the peer's V,
+    W and flag arrays, real peer stores from the step kernel's epilogue, real flag signals and waits.
+    The ranks time-share the GPU, so the barrier is host-sequenced (chase_filter_rows_hostsync_ws:
+    signal, stream sync, gloo barrier, wait) -- no kernel ever spins on a kernel of the other process."""
+    import os
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        torch.cuda.set_device(0)
+        dtype = getattr(torch, dtype_name)
+        w = W.make_config(2, N=N, ncols=n, dtype=dtype)
+        parts = sharding.row_partition(N, world, 128)
+        row0, nrows = parts[rank]
+        H_loc = _dev(w.H[row0:row0 + nrows, :])
+        f = sharding.RowShardedFilter(H_loc, row0, N, n, rank, world, host_barrier=dist.barrier)
+        f.V.copy_(w.V0)
+        f.W.fill_(float("nan"))
+        torch.cuda.synchronize()
+        dist.barrier()
+        f.run(w.degrees, w.a, w.b, w.lambda1)
+        torch.cuda.synchronize()
+        ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), w.degrees.numpy(), w.a, w.b, w.lambda1)
+        err = rel_fro(f.V.cpu().numpy(), ref)
+        flags = f.flags.cpu().numpy().tolist()
+        dist.barrier()
+        f.close()
+        q.put((rank, float(err), f.seq, flags))
+    except Exception as exc:       # surface the failure in the parent instead of a hang
+        q.put((rank, repr(exc), -1, []))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("dtype_name,N,n", [("complex128", 520, 77), ("float64", 1040, 150)])
+def test_row_sharded_filter_two_real_processes_on_one_gpu(dtype_name, N, n):
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29650 + (N % 97)
+    procs = [ctx.Process(target=_two_process_worker, args=(r, 2, port, N, n, dtype_name, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    results = []
+    try:
+        for _ in procs:
+            results.append(q.get(timeout=300))
+    finally:
+        for p in procs:
+            p.join(timeout=60)
+            if p.is_alive():
+                p.kill()
+    w = W.make_config(2, N=N, ncols=n, dtype=getattr(torch, dtype_name))
+    m_max = int(w.degrees.max())
+    assert sorted(r[0] for r in results) == [0, 1]
+    for rank, err, seq, flags in results:
+        assert isinstance(err, float), err
+        assert err <= 1e-12, (rank, err)
+        assert seq == 1 + m_max
+        assert flags[:2] == [seq, seq] and flags[2] == 0, flags      # both ranks' signals arrived; no timeout

@@ -190,6 +190,15 @@ def test_rows_and_lanczos_validation_rejects_before_any_launch():
     assert lib.chase_rows_barrier(None, peers, 2, 0, 1, None) == -1
     assert lib.chase_rows_barrier(0x6000, peers, 2, 5, 1, None) == -1
     assert lib.chase_rows_barrier(0x6000, peers, 17, 0, 1, None) == -1
+    assert lib.chase_rows_signal(0x6000, None, 2, 0, 1, None) == -1
+    assert lib.chase_rows_wait(None, 2, 1, None) == -1
+    assert lib.chase_rows_wait(0x6000, 0, 1, None) == -1
+    assert lib.chase_rows_status(None, 2, None) == -1
+    assert lib.chase_rows_status(0x6000, 17, None) == -1
+    cb = binding.HOST_BARRIER_FN(lambda _ctx: 0)
+    assert lib.chase_filter_rows_hostsync_ws(H, 64, 0, 32, X, 4, deg.ctypes.data, -1.0, 2.0, -2.0, 3, Y, 1 << 20,
+                                             1, 0, None, None, None, None, C.addressof(seq), None, cb, None) == -1   # host barrier without flags
+    assert rows_ws(degrees=np.asarray([2, 2, 4, 5000], dtype=np.int32)) == -3     # above CHASE_MAX_DEGREE
 
     al = np.zeros(10)
     def lanczos(N=64, nruns=2, k=5, dtype=3, ws=0x7000, ws_bytes=1 << 24, v0=X):
@@ -203,3 +212,26 @@ def test_rows_and_lanczos_validation_rejects_before_any_launch():
     assert lanczos(ws_bytes=1024) == -5
     assert lanczos(ws=0x7008) == -6
     assert pkg.chase_filter_launch_count() == before
+
+
+def test_parity_sample_plan_covers_every_degree_class_and_tile_edge():
+    """SURVEY 8(c): >= 32 columns; first / last column of every distinct degree; global first / last;
+    columns around the kernels' column-tile multiples; deterministic."""
+    from paper_1805_10121_b200 import workloads as W
+    for cfg in (3, 4, 5):
+        shape = W.CONFIG_SHAPES[cfg]
+        if cfg == 4:
+            deg = W.sorted_even_degrees(shape["ncols"], 8, 36, W.BASE_SEED + 4002)
+        else:
+            deg = W.uniform_degrees(shape["ncols"], 20 if cfg == 3 else 16)
+        cols = W.parity_sample_columns(deg)
+        assert cols == W.parity_sample_columns(deg)
+        assert cols == sorted(set(cols)) and len(cols) >= 32
+        assert cols[0] == 0 and cols[-1] == shape["ncols"] - 1
+        d = deg.numpy()
+        for v in np.unique(d):
+            idx = np.nonzero(d == v)[0]
+            assert idx[0] in cols and idx[-1] in cols
+        assert {63, 64, 65, 127, 128, 129} <= set(cols)
+    assert W.parity_sample_columns([]) == []
+    assert W.parity_sample_columns([2, 2, 4]) == [0, 1, 2]
