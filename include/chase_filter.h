@@ -70,8 +70,9 @@ enum {
 };
 
 /* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype` (the W of
- * Alg. 4), rounded up to 256 bytes (plus 256 bytes on the tcgen05 3xTF32 path, see
- * chase_filter_kernel_path: the counter of a soft barrier between the persistent CTAs).
+ * Alg. 4), rounded up to 256 bytes, plus -- see chase_filter_kernel_path -- 256 bytes on the tcgen05
+ * 3xTF32 path (the counter of a soft barrier between the persistent CTAs) or about 20 MB on the FP64
+ * tensor path (flags and partial accumulator tiles of the stream-K CTAs, chase_filter_step_plan).
  * 0 if an argument is invalid. */
 size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
@@ -84,7 +85,8 @@ size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtyp
  *              undefined on entry and exit
  *   stream     cudaStream_t
  * Enqueues exactly max(degrees) step kernels (plus one device copy per run of odd-degree
- * columns; on the 3xTF32 path a 4-byte memset before each kernel) and returns without synchronising. */
+ * columns; on the 3xTF32 path a 4-byte memset before each kernel, on the FP64 tensor path one 1 KB
+ * memset per call) and returns without synchronising. */
 int chase_filter_ws(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                     double a, double b, double lambda1, chase_dtype_t dtype,
                     void *workspace, size_t workspace_bytes, void *stream);
@@ -172,8 +174,24 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
  *   with g_sigma the Gaussian density of standard deviation sigma (paper default 0.25).
  *   nruns == 1 is the `approx` branch (l.4-5): only *b_sup is written (mu_1, mu_ne may be NULL).
  *   nev_nex is a double so that callers can aim between two eigenvalues; 0 < nev_nex < N.
- *   Returns 0 or CHASE_ERR_ARG (null pointer, bad size, non-finite / negative coefficient, sigma <= 0). */
+ *   Returns 0 or CHASE_ERR_ARG (null pointer, bad size, non-finite / negative coefficient, sigma <= 0).
+ *
+ * chase_lanczos_ritz_vectors (Alg. 6 l.13, explained at :471: "Since ZQ are the approximate
+ *   eigenvectors of A, we use those vectors corresponding to the Ritz values smaller than mu_{nev+nex} and
+ *   intersperse them with random i.i.d. vectors in V^"): for run `run` (the paper uses the first of the
+ *   n_vec runs, i.e. run = 1 when run 0 is the b_sup run), with T_k = Z^H diag(lam~) Z, writes the Ritz
+ *   vector  x_i = U^[run] z_i  of every Ritz value lam~_i < mu_ne, in ascending order of lam~_i and at
+ *   most max_vecs of them, into column dst_cols[i] of Vhat (DEVICE, N x ncols_vhat column-major) -- the
+ *   caller picks the columns, which is the interspersing.  The sign of x_i is fixed by Z_{1,i} >= 0.
+ *   `workspace` is the one a chase_lanczos call with the same (N, nruns, k, dtype) left behind (the
+ *   Lanczos vectors are still in it), alpha / beta that call's outputs (HOST [nruns * k]).
+ *   *count (HOST) receives the number of vectors written, ritz_values (HOST [max_vecs], may be NULL)
+ *   their Ritz values.  One N x k by k x count product in a small kernel; SYNCHRONISES `stream`. */
 size_t chase_lanczos_workspace_bytes(int64_t N, int64_t nruns, int32_t k, chase_dtype_t dtype);
+int chase_lanczos_ritz_vectors(const void *workspace, size_t workspace_bytes, int64_t N, int64_t nruns, int32_t k,
+                               chase_dtype_t dtype, int64_t run, const double *alpha, const double *beta,
+                               double mu_ne, void *Vhat, int64_t ncols_vhat, const int64_t *dst_cols,
+                               int64_t max_vecs, int64_t *count, double *ritz_values, void *stream);
 int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nruns, int32_t k, chase_dtype_t dtype,
                   double *alpha, double *beta, void *workspace, size_t workspace_bytes, void *stream);
 int chase_spectral_estimates(int32_t k, int64_t nruns, const double *alpha, const double *beta, int64_t N,
@@ -258,12 +276,17 @@ int chase_ipc_close(void *base);
  * into 0.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
-/* Column tiling the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active` columns
- * on a GPU with `sms` SMs (host only, no CUDA call; for tests and inspection).  out (HOST int32[4]) =
- * {row tiles of 128, column tiles of the full width (64 complex128 / 128 float64 columns), narrow
- * column tiles launched after them, width of a narrow tile}.  The tiles cover columns
- * [0, n_active) exactly once.  Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
-int chase_filter_step_tiling(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out);
+/* Work decomposition the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active`
+ * columns of an N x N problem on a GPU with `sms` SMs (host only, no CUDA call; for tests and inspection).
+ * out (HOST int32[6]) = {row tiles of 128, column tiles, column tile width, data-parallel tiles (one CTA
+ * each, grouped raster order), stream-K CTAs, k-slabs per tile}.  The column tiles cover [0, n_active)
+ * exactly once.  The tiles after the data-parallel ones are shared by the stream-K CTAs in contiguous
+ * k-slab ranges: sk_begin (HOST int32[stream-K CTAs + 1], at most CHASE_MAX_SK_CTAS + 1; may be NULL)
+ * receives the range boundaries, slab s being k-slab (s % slabs per tile) of tile (data-parallel tiles +
+ * s / slabs per tile).  Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
+#define CHASE_MAX_SK_CTAS 160
+int chase_filter_step_plan(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out,
+                           int32_t *sk_begin);
 
 /* Number of kernels launched by this library since load (all streams); for bench.py. */
 int64_t chase_filter_launch_count(void);

@@ -15,8 +15,11 @@ What the paper fixes and what it leaves open (readings G19-G22):
   * mu_{nev+nex} = t-bar with  int_{-inf}^{t-bar} phi~ = (nev+nex)/N   (l.11); "approximately" in the
     paper, here the exact root of the smooth, strictly increasing integral (G21).
   * mu_1 = min_j lambda~^[j]_1                                         (l.12)
-The random start vectors are INPUTS (the method's random draws are passed in).  Line 13
-(interspersing Ritz vectors into V^) only changes the caller's start block and is not covered (G22).
+  * l.13: "Z^[1] Q^[1]" are the approximate eigenvectors of A; Q^[1] is read as the
+    Lanczos basis U^[1] of the first DoS run (the paper's only other use of the letter; reading G22), so
+    the i-th Ritz vector is x_i = U^[1] z_i with z_i the eigenvector of T_k for lambda~_i.  Those with
+    lambda~_i < mu_{nev+nex} are returned, ascending; WHERE they go in V^ ("intersperse") is the caller's.
+The random start vectors are INPUTS (the method's random draws are passed in).
 """
 from __future__ import annotations
 
@@ -63,6 +66,21 @@ def ritz(alpha: np.ndarray, beta: np.ndarray):
         T[j, j + 1] = T[j + 1, j] = beta[j]
     lam, Z = np.linalg.eigh(T)
     return lam, Z[0, :] ** 2
+
+
+def ritz_vectors(U: np.ndarray, alpha: np.ndarray, beta: np.ndarray, mu_ne: float):
+    """Alg. 6 l.13: Ritz pairs (lam~_i, x_i = U z_i) of one Lanczos run with
+    lam~_i < mu_ne, ascending in lam~_i.  T_k z_i = lam~_i z_i by the dense symmetric eigensolver; the
+    sign of z_i is fixed by a non-negative first component (it is never zero for beta_j > 0).
+    Returns (lam [m], X [N, m], last components |Z_{k,i}| [m])."""
+    k = len(alpha)
+    T = np.diag(np.asarray(alpha, dtype=np.float64))
+    for j in range(k - 1):
+        T[j, j + 1] = T[j + 1, j] = beta[j]
+    lam, Z = np.linalg.eigh(T)                       # columns of Z: eigenvectors, lam ascending
+    Z = Z * np.where(Z[0, :] < 0.0, -1.0, 1.0)[None, :]
+    sel = np.nonzero(lam < mu_ne)[0]
+    return lam[sel], U @ Z[:, sel], np.abs(Z[k - 1, sel])
 
 
 def normal_cdf(x: float) -> float:

@@ -21,8 +21,8 @@ EXPORTS = [
     "chase_filter", "chase_filter_ws", "chase_filter_host", "chase_filter_workspace_bytes",
     "chase_filter_scalars", "chase_filter_schedule", "chase_filter_kernel_path",
     "chase_filter_launch_count", "chase_fp64_peak_probe", "chase_filter_strerror", "chase_degrees",
-    "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_tiling",
-    "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates",
+    "chase_hemm", "chase_residuals", "chase_residuals_workspace_bytes", "chase_filter_step_plan",
+    "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates", "chase_lanczos_ritz_vectors",
     "chase_hemm_rows", "chase_rows_barrier", "chase_rows_signal", "chase_rows_wait", "chase_rows_status",
     "chase_filter_rows_ws", "chase_filter_rows_hostsync_ws", "chase_ipc_export", "chase_ipc_open",
     "chase_ipc_close",
@@ -81,12 +81,15 @@ def load() -> ctypes.CDLL:
     lib.chase_residuals_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
     lib.chase_residuals.restype = ctypes.c_int
     lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
-    lib.chase_filter_step_tiling.restype = ctypes.c_int
-    lib.chase_filter_step_tiling.argtypes = [i64, i64, ctypes.c_int, i32, vp]
+    lib.chase_filter_step_plan.restype = ctypes.c_int
+    lib.chase_filter_step_plan.argtypes = [i64, i64, ctypes.c_int, i32, vp, vp]
     lib.chase_lanczos_workspace_bytes.restype = sz
     lib.chase_lanczos_workspace_bytes.argtypes = [i64, i64, i32, ctypes.c_int]
     lib.chase_lanczos.restype = ctypes.c_int
     lib.chase_lanczos.argtypes = [vp, i64, vp, i64, i32, ctypes.c_int, vp, vp, vp, sz, vp]
+    lib.chase_lanczos_ritz_vectors.restype = ctypes.c_int
+    lib.chase_lanczos_ritz_vectors.argtypes = [vp, sz, i64, i64, i32, ctypes.c_int, i64, vp, vp, dbl, vp, i64, vp, i64,
+                                               vp, vp, vp]
     lib.chase_spectral_estimates.restype = ctypes.c_int
     lib.chase_spectral_estimates.argtypes = [i32, i64, vp, vp, i64, dbl, dbl, vp, vp, vp]
     lib.chase_hemm_rows.restype = ctypes.c_int
@@ -245,11 +248,17 @@ def chase_filter_schedule(degrees: Sequence[int]):
     return m_max, offset
 
 
-def chase_filter_step_tiling(N: int, n_active: int, dtype: torch.dtype, sms: int = 148):
-    """(row tiles, full-width column tiles, narrow column tiles, narrow tile width) of one launch."""
-    out = np.zeros(4, dtype=np.int32)
-    _check(load().chase_filter_step_tiling(int(N), int(n_active), _DTYPE_CODE[dtype], int(sms), out.ctypes.data))
-    return tuple(int(x) for x in out)
+def chase_filter_step_plan(N: int, n_active: int, dtype: torch.dtype, sms: int = 148):
+    """Work decomposition of one FP64 tensor-kernel launch: dict with tiles_m, tiles_n, tile_width,
+    dp_tiles, sk_ctas, slabs_per_tile and sk_begin (numpy int32[sk_ctas + 1])."""
+    out = np.zeros(6, dtype=np.int32)
+    skb = np.zeros(161, dtype=np.int32)
+    _check(load().chase_filter_step_plan(int(N), int(n_active), _DTYPE_CODE[dtype], int(sms), out.ctypes.data,
+                                         skb.ctypes.data))
+    keys = ("tiles_m", "tiles_n", "tile_width", "dp_tiles", "sk_ctas", "slabs_per_tile")
+    plan = {k: int(v) for k, v in zip(keys, out)}
+    plan["sk_begin"] = skb[: plan["sk_ctas"] + 1].copy()
+    return plan
 
 
 def chase_fp64_peak_probe(kind: int, iters: int = 4096) -> float:
@@ -346,6 +355,34 @@ def chase_lanczos(H: torch.Tensor, V0: torch.Tensor, k: int, workspace: Optional
                                     alpha.ctypes.data, beta.ctypes.data, workspace.data_ptr(),
                                     workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
     return alpha, beta
+
+
+def chase_lanczos_ritz_vectors(workspace: torch.Tensor, N: int, dtype: torch.dtype, alpha, beta, run: int,
+                               mu_ne: float, Vhat: torch.Tensor, dst_cols,
+                               stream: Optional[torch.cuda.Stream] = None):
+    """Alg. 6 l.13: Ritz vectors of run `run` with Ritz value < mu_ne (ascending) into the columns
+    dst_cols[i] of Vhat; `workspace` / alpha / beta come from the chase_lanczos call.  Returns the Ritz
+    values written (numpy, length = number of vectors written <= len(dst_cols))."""
+    if not (workspace.is_cuda and Vhat.is_cuda) or Vhat.dtype != dtype or dtype not in _DTYPE_CODE:
+        raise ValueError("workspace and Vhat must be CUDA tensors, Vhat of the Lanczos dtype")
+    _check_colmajor(Vhat, "Vhat")
+    if Vhat.shape[0] != N:
+        raise ValueError("Vhat must have N rows")
+    a = np.ascontiguousarray(np.asarray(alpha, dtype=np.float64))
+    b = np.ascontiguousarray(np.asarray(beta, dtype=np.float64))
+    if a.ndim != 2 or a.shape != b.shape:
+        raise ValueError("alpha and beta must be [nruns, k] arrays of equal shape")
+    nruns, k = a.shape
+    dst = np.ascontiguousarray(np.asarray(dst_cols, dtype=np.int64))
+    count = ctypes.c_int64()
+    vals = np.zeros(max(dst.size, 1), dtype=np.float64)
+    with torch.cuda.device(Vhat.device):
+        _check(load().chase_lanczos_ritz_vectors(
+            workspace.data_ptr(), workspace.numel() * workspace.element_size(), int(N), int(nruns), int(k),
+            _DTYPE_CODE[dtype], int(run), a.ctypes.data, b.ctypes.data, float(mu_ne), Vhat.data_ptr(),
+            int(Vhat.shape[1]), dst.ctypes.data, int(dst.size), ctypes.addressof(count), vals.ctypes.data,
+            _stream_ptr(stream)))
+    return vals[: int(count.value)].copy()
 
 
 def chase_spectral_estimates(alpha, beta, N: int, nev_nex: float, sigma: float = 0.25):

@@ -52,7 +52,9 @@ size_t chase_filter_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtyp
     size_t w = elem_bytes(dtype);
     if (w == 0 || N <= 0 || ncols < 0 || N > kMaxDim || ncols > kMaxDim) return 0;
     size_t bytes = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
-    if (chase_filter_kernel_path(N, ncols, dtype) == 2) bytes += 256;   // tcgen05 path: soft grid barrier counter
+    const int path = chase_filter_kernel_path(N, ncols, dtype);
+    if (path == 2) bytes += 256;                         // tcgen05 path: soft grid barrier counter
+    if (path == 1) bytes += dmma_sk_scratch_bytes();     // FP64 tensor path: stream-K flags + partial tiles
     return bytes;
 }
 
@@ -142,7 +144,7 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
 namespace chase {
 int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha,
                            double beta, double c, const double *c_col, int use_beta, chase_dtype_t dtype,
-                           cudaStream_t stream) {
+                           cudaStream_t stream, void *sk_scratch) {
     const int path = chase_filter_kernel_path(N, ncols, dtype);
     const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
     // A few vectors: one streaming pass over H.  In FP64 the narrow-tile DMMA kernel is the faster
@@ -158,6 +160,7 @@ int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t nc
         DmmaPlan plan;
         cudaError_t e = dmma_plan_create(&plan, dtype, H, N, const_cast<void *>(X), Y, ncols);
         if (e != cudaSuccess) return (int)e;
+        plan.sk_scratch = sk_scratch;       // null: stream-ordered memory for this one launch
         e = dmma_launch_step(&plan, 0, 0, alpha, beta, c, use_beta, stream, c_col);
         return (int)e;
     }
@@ -214,7 +217,9 @@ int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, cons
     // a pinned one is read in stream order (see the header): no synchronisation either way.
     cudaError_t e = cudaMemcpyAsync(d_shift, ritzv, (size_t)ncols * sizeof(double), cudaMemcpyHostToDevice, stream);
     if (e != cudaSuccess) return (int)e;
-    int rc = launch_one_step(H, N, V, workspace, ncols, 1.0, 0.0, 0.0, d_shift, 0, dtype, stream);
+    const size_t vb = ((size_t)N * (size_t)ncols * elem_bytes(dtype) + 255) / 256 * 256;
+    void *sk = chase_filter_kernel_path(N, ncols, dtype) == 1 ? (char *)workspace + vb : nullptr;
+    int rc = launch_one_step(H, N, V, workspace, ncols, 1.0, 0.0, 0.0, d_shift, 0, dtype, stream, sk);
     if (rc != CHASE_OK) return rc;
     return (int)launch_column_norms(dtype, workspace, N, ncols, resid, stream);
 }
@@ -235,6 +240,34 @@ int chase_lanczos(const void *H, int64_t N, const void *V0, int64_t nvec, int32_
     if (((uintptr_t)H | (uintptr_t)V0 | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
     try {
         return (int)lanczos_run(H, N, V0, (int)nvec, k, dtype, w, workspace, alpha, beta, (cudaStream_t)stream_);
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
+    }
+}
+
+int chase_lanczos_ritz_vectors(const void *workspace, size_t workspace_bytes, int64_t N, int64_t nruns, int32_t k,
+                               chase_dtype_t dtype, int64_t run, const double *alpha, const double *beta,
+                               double mu_ne, void *Vhat, int64_t ncols_vhat, const int64_t *dst_cols,
+                               int64_t max_vecs, int64_t *count, double *ritz_values, void *stream_) {
+    const size_t w = elem_bytes(dtype);
+    if (w == 0) return CHASE_ERR_DTYPE;
+    if (N <= 0 || nruns <= 0 || k <= 0 || N > kMaxDim || nruns > 4096 || k > 4096 || k > N) return CHASE_ERR_ARG;
+    if (run < 0 || run >= nruns || !alpha || !beta || !count || !std::isfinite(mu_ne)) return CHASE_ERR_ARG;
+    if (max_vecs < 0 || ncols_vhat < 0 || ncols_vhat > kMaxDim || (max_vecs > 0 && (!Vhat || !dst_cols))) return CHASE_ERR_ARG;
+    for (int64_t i = 0; i < max_vecs; ++i)
+        if (dst_cols[i] < 0 || dst_cols[i] >= ncols_vhat) return CHASE_ERR_ARG;
+    for (int32_t j = 0; j < k; ++j) {
+        const double al = alpha[run * k + j], be = beta[run * k + j];
+        if (!std::isfinite(al) || !std::isfinite(be) || be < 0.0) return CHASE_ERR_ARG;
+    }
+    if (!workspace || workspace_bytes < lanczos_workspace_bytes(N, nruns, k, w)) return CHASE_ERR_WORKSPACE;
+    if (((uintptr_t)workspace | (uintptr_t)Vhat) & 15) return CHASE_ERR_ALIGN;
+    *count = 0;
+    if (max_vecs == 0) return CHASE_OK;
+    try {
+        return (int)lanczos_ritz_vectors(workspace, N, (int)nruns, k, dtype, w, (int)run, alpha + run * k, beta + run * k,
+                                         mu_ne, Vhat, dst_cols, std::min<int64_t>(max_vecs, k), count, ritz_values,
+                                         (cudaStream_t)stream_);
     } catch (const std::exception &) {
         return (int)cudaErrorMemoryAllocation;
     }
@@ -297,11 +330,20 @@ int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     return 0;
 }
 
-int chase_filter_step_tiling(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out) {
+int chase_filter_step_plan(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out,
+                           int32_t *sk_begin) {
     if (elem_bytes(dtype) == 0) return CHASE_ERR_DTYPE;
     if (N <= 0 || n_active <= 0 || N > kMaxDim || n_active > kMaxDim || sms <= 0 || !out) return CHASE_ERR_ARG;
     if (dtype != CHASE_C128 && dtype != CHASE_F64) return CHASE_ERR_DTYPE;
-    dmma_plan_tiling(N, n_active, dtype, sms, out);
+    StepPlan pl;
+    try {
+        dmma_step_plan(N, n_active, dtype, sms, &pl);
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
+    }
+    out[0] = pl.tiles_m; out[1] = pl.tiles_n; out[2] = pl.bn_w; out[3] = pl.dp_tiles; out[4] = pl.sk_ctas; out[5] = pl.KT;
+    if (sk_begin)
+        for (int g = 0; g <= pl.sk_ctas; ++g) sk_begin[g] = pl.sk_begin[g];
     return CHASE_OK;
 }
 
@@ -367,6 +409,7 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
     if (use_dmma) {
         cudaError_t e = dmma_plan_create(&plan, dtype, H, N, V, workspace, ncols);
         if (e != cudaSuccess) return (int)e;
+        plan.sk_scratch = (char *)workspace + ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
     }
     if (use_tf32) {
         const size_t vb = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;

@@ -32,6 +32,20 @@ constexpr int kSkinnyMaxCols = 8;
 cudaError_t launch_step_skinny(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
 
 // TMA + DMMA tensor kernels (CHASE_C128 with any N >= 16, CHASE_F64 with even N).
+// Work decomposition of one launch on `n` active columns (csrc/step_dmma.cu): tiles of
+// 128 rows x bn_w columns in grouped raster order; the first dp_tiles tiles get one CTA each, the k-slabs
+// of the remaining tiles are shared by sk_ctas stream-K CTAs: CTA g owns slabs [sk_begin[g], sk_begin[g+1])
+// of that region, slab s = k-slab (s % KT) of tile dp_tiles + s / KT.
+constexpr int kMaxSkCtas = 160;                 // >= SM count of any sm_100 part
+constexpr size_t kSkFlagBytes = 1024;           // kMaxSkCtas uint32 flags, padded
+struct StepPlan {
+    int KT, tiles_m, tiles_n, bn_w, dp_tiles, sk_ctas;
+    int sk_begin[kMaxSkCtas + 1];
+};
+// Bytes of device scratch the stream-K CTAs need (flags + one partial accumulator tile per CTA).
+size_t dmma_sk_scratch_bytes();
+void dmma_step_plan(int64_t N, int64_t n, chase_dtype_t dtype, int sms, StepPlan *out);
+
 // A plan holds the three tensor maps (H, and both vector buffers) of one chase_filter call.
 struct DmmaPlan {
     alignas(64) unsigned char tmap_H[128];
@@ -45,11 +59,13 @@ struct DmmaPlan {
     void *buf[2];
     int npeers;                                 // row-sharded: peer-mapped copies of buf[0], buf[1] on the other GPUs
     void *peer_buf[2][CHASE_MAX_RANKS - 1];
+    void *sk_scratch;                           // dmma_sk_scratch_bytes() of device memory, or null: every launch that
+                                                // needs it then takes stream-ordered memory (cudaMallocAsync)
+    uint32_t sk_epoch;                          // flag value of the last stream-K launch on sk_scratch (0: flags not yet zeroed)
+    int64_t step_plan_n;                        // active width step_plan was made for (-1: none)
+    StepPlan step_plan;
 };
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
-// Column tiling one launch on `n` active columns would use on `sms` SMs:
-// out = {row tiles, full-width column tiles, narrow column tiles, narrow tile width}.
-void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_t out[4]);
 // Returns cudaSuccess, or an error (then the caller falls back to the generic kernels
 // only if the failure is "driver entry point unavailable"; anything else is reported).
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N,
@@ -62,7 +78,7 @@ cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const voi
 cudaError_t dmma_plan_create_panel(DmmaPlan *plan, chase_dtype_t dtype, const void *H_full, int64_t N, int64_t row0,
                                    int64_t nrows, void *V, void *W, int64_t ncols);
 // Step reading buffer `src` (0/1) and writing buffer 1-src, active columns [s, ncols).
-cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
+cudaError_t dmma_launch_step(DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
                              double c, int use_beta, cudaStream_t stream, const double *c_col = nullptr);
 
 // tcgen05 3xTF32 kernels (CHASE_C64 with N % 2 == 0, CHASE_F32 with N % 4 == 0).
@@ -93,13 +109,20 @@ cudaError_t launch_column_norms(chase_dtype_t dtype, const void *R, int64_t N, i
 // One launch of the step kernel family on whole buffers: Y <- alpha (H X - c X) + beta Y (c_col: optional
 // per-column shift).  Returns 0, a negative CHASE_ERR_* or a positive cudaError_t.
 int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t ncols, double alpha, double beta,
-                    double c, const double *c_col, int use_beta, chase_dtype_t dtype, cudaStream_t stream);
+                    double c, const double *c_col, int use_beta, chase_dtype_t dtype, cudaStream_t stream,
+                    void *sk_scratch = nullptr);
 
 // Alg. 6: 1 + n_vec coalesced Lanczos runs (csrc/lanczos.cu).  alpha_host / beta_host: HOST [nvec * k],
 // run r at offset r * k.  Synchronises `stream`.
 size_t lanczos_workspace_bytes(int64_t N, int64_t nvec, int32_t k, size_t elem);
 cudaError_t lanczos_run(const void *H, int64_t N, const void *V0, int nvec, int k, chase_dtype_t dtype, size_t elem,
                         void *workspace, double *alpha_host, double *beta_host, cudaStream_t stream);
+// Alg. 6 l.13: Ritz vectors U^[run] z_i of the run's Ritz values below mu_ne (ascending, at most max_vecs) into
+// columns dst_cols[i] of Vhat; `workspace` is the one lanczos_run left behind.  Synchronises `stream`.
+cudaError_t lanczos_ritz_vectors(const void *workspace, int64_t N, int nvec, int k, chase_dtype_t dtype, size_t elem,
+                                 int run, const double *alpha_run, const double *beta_run, double mu_ne, void *Vhat,
+                                 const int64_t *dst_cols, int64_t max_vecs, int64_t *count, double *ritz_values,
+                                 cudaStream_t stream);
 // Ritz values (unsorted) and squared first eigenvector components of T_k; false = QL did not converge.
 bool lanczos_ritz(int k, const double *alpha, const double *beta, std::vector<double> &lam, std::vector<double> &w);
 

@@ -9,6 +9,7 @@
 //
 // Reading G19: full re-orthogonalisation by two passes of classical Gram-Schmidt against
 // all previous Lanczos vectors; alpha_j is the j-th coefficient of the first pass.
+#include <algorithm>
 #include <cmath>
 #include <vector>
 
@@ -147,14 +148,15 @@ cudaError_t run(const void *H, int64_t N, const void *V0, int nvec, int k, chase
     return cudaGetLastError();
 }
 
-// Eigenvalues of the symmetric tridiagonal T (diagonal d[0..n), off-diagonal e[0..n-1)) and the FIRST
-// components of its normalised eigenvectors, by the implicit-shift QL iteration with the rotations
-// applied to the row vector z = e_1^T only (Golub-Welsch).  On return d holds the eigenvalues
-// (unsorted), z the first components.  Returns false if an eigenvalue needs more than 60 sweeps.
-bool tridiag_ql_first_row(int n, std::vector<double> &d, std::vector<double> &e, std::vector<double> &z) {
+// Eigenvalues of the symmetric tridiagonal T (diagonal d[0..n), off-diagonal e[0..n-1)) and the first
+// `zrows` ROWS of its normalised eigenvector matrix, by the implicit-shift QL iteration with the
+// rotations applied to those rows of the identity (zrows = 1: Golub-Welsch, only the first components;
+// zrows = n: all eigenvectors, column i belonging to d[i]).  On return d holds the eigenvalues
+// (unsorted), z (row-major zrows x n) the rows.  Returns false if an eigenvalue needs more than 60 sweeps.
+bool tridiag_ql(int n, std::vector<double> &d, std::vector<double> &e, std::vector<double> &z, int zrows) {
     e.resize(n, 0.0);
-    z.assign(n, 0.0);
-    z[0] = 1.0;
+    z.assign((size_t)zrows * n, 0.0);
+    for (int r = 0; r < zrows; ++r) z[(size_t)r * n + r] = 1.0;
     const double eps = 2.220446049250313e-16;
     for (int l = 0; l < n; ++l) {
         int iter = 0, m;
@@ -187,9 +189,12 @@ bool tridiag_ql_first_row(int n, std::vector<double> &d, std::vector<double> &e,
                     p = s * r;
                     d[i + 1] = g + p;
                     g = c * r - b;
-                    f = z[i + 1];
-                    z[i + 1] = s * z[i] + c * f;
-                    z[i] = c * z[i] - s * f;
+                    for (int row = 0; row < zrows; ++row) {
+                        double *zr = &z[(size_t)row * n];
+                        f = zr[i + 1];
+                        zr[i + 1] = s * zr[i] + c * f;
+                        zr[i] = c * zr[i] - s * f;
+                    }
                 }
                 if (r == 0.0 && i >= l) continue;
                 d[l] -= p;
@@ -201,13 +206,33 @@ bool tridiag_ql_first_row(int n, std::vector<double> &d, std::vector<double> &e,
     return true;
 }
 
+// Vhat[:, dst[i]] = sum_j U_j[:, run] S[j, i]: the Ritz vectors U^[run] z_i of Alg. 6 l.13 (S = the selected
+// eigenvectors of T_k, k x cnt column-major, real).  One thread per (row, output vector).
+template <typename T>
+__global__ void __launch_bounds__(kBlock) lz_ritz_vectors(const T *__restrict__ U, int64_t N, int nvec, int run, int k,
+                                                          const double *__restrict__ S, T *__restrict__ Vhat,
+                                                          const int64_t *__restrict__ dst) {
+    const int i = blockIdx.y;
+    const int64_t r = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+    if (r >= N) return;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int j = 0; j < k; ++j) {
+        const double2 u = ld(U + ((int64_t)j * nvec + run) * N, r);
+        const double sji = S[(int64_t)i * k + j];
+        acc.x = fma(sji, u.x, acc.x);
+        acc.y = fma(sji, u.y, acc.y);
+    }
+    st(Vhat + dst[i] * N, r, acc);
+}
+
 }  // namespace
 
 size_t lanczos_workspace_bytes(int64_t N, int64_t nvec, int32_t k, size_t elem) {
     const size_t vec = (size_t)N * (size_t)nvec * elem;
     return round256(vec * (size_t)k) + round256(vec)                      // U (k blocks), w
            + 2 * round256((size_t)nvec * k * sizeof(double))              // alpha, beta
-           + round256((size_t)nvec * k * sizeof(double2));                // Gram-Schmidt coefficients
+           + round256((size_t)nvec * k * sizeof(double2))                 // Gram-Schmidt coefficients
+           + round256((size_t)k * k * sizeof(double)) + round256((size_t)k * sizeof(int64_t));   // Ritz-vector coefficients, targets
 }
 
 cudaError_t lanczos_run(const void *H, int64_t N, const void *V0, int nvec, int k, chase_dtype_t dtype, size_t elem,
@@ -231,9 +256,52 @@ cudaError_t lanczos_run(const void *H, int64_t N, const void *V0, int nvec, int 
     return cudaStreamSynchronize(stream);
 }
 
+cudaError_t lanczos_ritz_vectors(const void *workspace, int64_t N, int nvec, int k, chase_dtype_t dtype, size_t elem,
+                                 int run, const double *alpha_run, const double *beta_run, double mu_ne, void *Vhat,
+                                 const int64_t *dst_cols, int64_t max_vecs, int64_t *count, double *ritz_values,
+                                 cudaStream_t stream) {
+    // T_k = Z^H diag(lam) Z on the host (k x k, negligible: PAPER.md:473)
+    std::vector<double> d(alpha_run, alpha_run + k), e(beta_run, beta_run + (k > 0 ? k - 1 : 0)), z;
+    if (!tridiag_ql(k, d, e, z, k)) return cudaErrorInvalidValue;
+    std::vector<int> order(k);
+    for (int i = 0; i < k; ++i) order[i] = i;
+    std::sort(order.begin(), order.end(), [&](int x, int y) { return d[x] < d[y]; });
+    std::vector<double> S;
+    int64_t cnt = 0;
+    for (int oi = 0; oi < k && cnt < max_vecs; ++oi) {
+        const int i = order[oi];
+        if (!(d[i] < mu_ne)) break;                                       // l.13: Ritz values below mu_{nev+nex}
+        const double sgn = z[(size_t)0 * k + i] < 0.0 ? -1.0 : 1.0;       // unique sign: first component >= 0
+        for (int j = 0; j < k; ++j) S.push_back(sgn * z[(size_t)j * k + i]);
+        if (ritz_values) ritz_values[cnt] = d[i];
+        ++cnt;
+    }
+    *count = cnt;
+    if (cnt == 0) return cudaSuccess;
+    const size_t vec = (size_t)N * (size_t)nvec * elem;
+    char *base = (char *)const_cast<void *>(workspace);
+    char *p = base + round256(vec * (size_t)k) + round256(vec) + 2 * round256((size_t)nvec * k * sizeof(double)) +
+              round256((size_t)nvec * k * sizeof(double2));
+    double *d_S = (double *)p;
+    int64_t *d_dst = (int64_t *)(p + round256((size_t)k * k * sizeof(double)));
+    cudaError_t err;
+    if ((err = cudaMemcpyAsync(d_S, S.data(), S.size() * sizeof(double), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return err;
+    if ((err = cudaMemcpyAsync(d_dst, dst_cols, (size_t)cnt * sizeof(int64_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return err;
+    if ((err = cudaStreamSynchronize(stream)) != cudaSuccess) return err;   // S is a local: consumed before return
+    const dim3 grid((unsigned)((N + kBlock - 1) / kBlock), (unsigned)cnt);
+    switch (dtype) {
+        case CHASE_F32:  lz_ritz_vectors<float><<<grid, kBlock, 0, stream>>>((const float *)workspace, N, nvec, run, k, d_S, (float *)Vhat, d_dst); break;
+        case CHASE_F64:  lz_ritz_vectors<double><<<grid, kBlock, 0, stream>>>((const double *)workspace, N, nvec, run, k, d_S, (double *)Vhat, d_dst); break;
+        case CHASE_C64:  lz_ritz_vectors<float2><<<grid, kBlock, 0, stream>>>((const float2 *)workspace, N, nvec, run, k, d_S, (float2 *)Vhat, d_dst); break;
+        default:         lz_ritz_vectors<double2><<<grid, kBlock, 0, stream>>>((const double2 *)workspace, N, nvec, run, k, d_S, (double2 *)Vhat, d_dst); break;
+    }
+    count_launch();
+    return cudaGetLastError();
+}
+
 bool lanczos_ritz(int k, const double *alpha, const double *beta, std::vector<double> &lam, std::vector<double> &w) {
     std::vector<double> d(alpha, alpha + k), e(beta, beta + (k > 0 ? k - 1 : 0)), z;
-    if (!tridiag_ql_first_row(k, d, e, z)) return false;
+    if (!tridiag_ql(k, d, e, z, 1)) return false;
     lam = d;
     w.resize(k);
     for (int i = 0; i < k; ++i) w[i] = z[i] * z[i];

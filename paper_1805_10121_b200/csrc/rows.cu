@@ -175,8 +175,7 @@ int chase_filter_rows_hostsync_ws(const void *H_loc, int64_t N, int64_t row0, in
     if (m_max < 0) return m_max;
     if (ncols == 0 || m_max == 0) return CHASE_OK;
     const size_t w = elem_size(dtype);
-    const size_t vb = ((size_t)N * (size_t)ncols * w + 255) / 256 * 256;
-    if (!workspace || workspace_bytes < vb) return CHASE_ERR_WORKSPACE;
+    if (!workspace || workspace_bytes < (size_t)N * (size_t)ncols * w) return CHASE_ERR_WORKSPACE;   // one vector block
     if (((uintptr_t)H_loc | (uintptr_t)V | (uintptr_t)workspace) & 15) return CHASE_ERR_ALIGN;
 
     int32_t offset[CHASE_MAX_DEGREE + 1];

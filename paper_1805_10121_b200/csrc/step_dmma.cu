@@ -18,11 +18,24 @@
 // The k index each MMA lane slot consumes is a free permutation; it is chosen so that every
 // fragment load is bank-conflict free under the swizzle (complex: k = 8q + 2t + a; real:
 // k = {0,10,4,14}[t] ^ a with 16-byte loads shared by two MMAs), identically for A and B.
+//
+// Work decomposition of one launch (DESIGN.md 6.1 "stream-K tail"): the first `dp_tiles` CTAs own one
+// whole output tile each (data-parallel, grouped raster); the last `sk_ctas` CTAs share the remaining
+// tiles' k-slabs in equal-TIME contiguous ranges (stream-K): a CTA whose range ends inside a tile
+// leaves its partial accumulators in the scratch buffer and raises a flag, the CTA that reaches the
+// tile's last slab adds the partials of the lower-numbered CTAs and runs the fused epilogue.  A CTA
+// only ever waits on CTAs with a smaller blockIdx, which were dispatched before it.
+// Launched with programmatic stream serialisation: prologue and the first H loads of step k+1
+// overlap the tail of step k (griddepcontrol).
 #include <cuda.h>
 
 #include <algorithm>
 #include <cmath>
+#include <cstring>
+#include <exception>
+#include <functional>
 #include <mutex>
+#include <queue>
 #include <vector>
 
 #include "chase_internal.h"
@@ -106,6 +119,9 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
 
 // ---------------------------------------------------------------- the kernel
 constexpr int kMaxPeers = CHASE_MAX_RANKS - 1;
+constexpr int kConsumerThreads = kConsumerWarps * 32;
+constexpr int kPartBytes = 128 * 1024;     // one partial accumulator tile: 256 threads x 64 doubles (both dtypes)
+
 struct StepParams {
     const double *X;     // source iterate V_k, first ACTIVE column (ld = N elements)
     double *Y;           // destination (holds V_{k-1}, becomes V_{k+1}), first active column
@@ -117,13 +133,18 @@ struct StepParams {
     double *peer_Y[kMaxPeers];   // peer-mapped pointers, already offset to the first active column
     int n;               // active columns
     int col0;            // first active column in the full buffer (TMA coordinate offset)
-    int tiles_m;
-    int tiles_wide;      // column tiles of the full width BN, covering columns [0, tiles_wide * BN)
-    int tiles_narrow;    // column tiles of width narrow_w covering the remaining columns
-    int narrow_w;        // multiple of 8 * WARPS_N, <= BN
+    int tiles_m, tiles_n;
+    int bn_w;            // column tile width of this launch: a multiple of 8 * WARPS_N, <= BN
+    int dp_tiles;        // tiles [0, dp_tiles) in raster order: one CTA each
+    int sk_ctas;         // stream-K CTAs covering tiles [dp_tiles, tiles_m * tiles_n)
+    uint32_t epoch;      // value the stream-K flags take in this launch
+    unsigned char *sk_part;   // sk_ctas partial tiles of kPartBytes
+    uint32_t *sk_flag;        // sk_ctas flags
     double alpha, beta, c;
     const double *c_col;   // optional per-column shift (device, indexed by active column); overrides c
     int use_beta;
+    int sk_begin[kMaxSkCtas + 1];   // CTA g owns the slabs [sk_begin[g], sk_begin[g+1]) of the stream-K region,
+                                    // slab s = k-slab (s % KT) of tile dp_tiles + s / KT
 };
 
 // Grouped rasterisation: consecutive CTAs cover kGroupN column tiles x a run of row tiles, so the
@@ -131,23 +152,23 @@ struct StepParams {
 // so that a wave of 148 CTAs is roughly square in BYTES (rows*BM ~ cols*BN), which minimises the
 // DRAM traffic of 148 register-resident output tiles.
 template <int kGroupN>
-__device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
+__host__ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
     const int per_group = kGroupN * tiles_m;
     const int grp = t / per_group;
     const int first_n = grp * kGroupN;
-    const int gn = min(kGroupN, tiles_n - first_n);
+    const int gn = (tiles_n - first_n) < kGroupN ? (tiles_n - first_n) : kGroupN;
     const int r = t - grp * per_group;
     tm = r / gn;
     tn = first_n + r % gn;
 }
 
-// The k loop of one consumer warp.  FULL = every 8-column block of the warp is valid (the common
-// case: no per-block test, so the compiler schedules loads and MMAs across blocks); otherwise only
-// the first jmax blocks are computed (ragged / narrow tiles).
+// The k loop of one consumer warp over `len` slabs, ring position `it` onwards.  FULL = every 8-column
+// block of the warp is valid (the common case: no per-block test, so the compiler schedules loads and
+// MMAs across blocks); otherwise only the first jmax blocks are computed (ragged / narrow tiles).
 template <bool CPLX, bool FULL>
 __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::WM / 8][Cfg<CPLX>::WN / 8][2],
-                                         const unsigned char *smem, uint32_t bar_base, int KT, int lane, int warp,
-                                         int jmax) {
+                                         const unsigned char *smem, uint32_t bar_base, uint32_t it, int len, int lane,
+                                         int warp, int jmax) {
     using C = Cfg<CPLX>;
     using S = Smem<CPLX>;
     constexpr int BN = C::BN, BK = C::BK, STAGES = C::STAGES;
@@ -169,9 +190,9 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
         if ((a & 1) == 0) real_b_off[a >> 1] = g * 128 + ((((kl >> 1) & 7) ^ g) << 4);
     }
 
-    for (int kt = 0; kt < KT; ++kt) {
-        const int s = kt % STAGES;
-        mbar_wait(bar_base + 8 * s, (kt / STAGES) & 1);
+    uint32_t s = it % STAGES, ph = (it / STAGES) & 1;
+    for (int kt = 0; kt < len; ++kt) {
+        mbar_wait(bar_base + 8 * s, ph);
         const unsigned char *sa = smem + s * S::STAGE_BYTES;
         const unsigned char *sb = sa + S::A_BYTES;
 
@@ -246,14 +267,36 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_base + 8 * (STAGES + s));
+        if (++s == STAGES) { s = 0; ph ^= 1; }
     }
+}
 
+// One unit of a CTA's work: k-slabs [k0, k1) of output tile `tile` (raster index).
+struct Segment {
+    int tile, k0, k1;
+};
+// Segment `idx` of this CTA (DP CTAs have exactly one); false when the CTA's work is exhausted.
+// `s` walks the CTA's slab range of the stream-K region.
+__device__ __forceinline__ bool next_segment(const StepParams &p, int KT, bool is_dp, int &s, int s_end, Segment &seg) {
+    if (is_dp) {
+        if (s != 0) return false;
+        seg.tile = blockIdx.x; seg.k0 = 0; seg.k1 = KT;
+        s = 1;
+        return true;
+    }
+    if (s >= s_end) return false;
+    const int tr = s / KT;
+    seg.tile = p.dp_tiles + tr;
+    seg.k0 = s - tr * KT;
+    seg.k1 = min(KT, seg.k0 + (s_end - s));
+    s += seg.k1 - seg.k0;
+    return true;
 }
 
 template <bool CPLX>
 __global__ void __launch_bounds__(kThreads, 1)
 step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
-                 const StepParams p) {
+                 const __grid_constant__ StepParams p) {
     using C = Cfg<CPLX>;
     using S = Smem<CPLX>;
     constexpr int BM = C::BM, BN = C::BN, BK = C::BK, STAGES = C::STAGES;
@@ -266,27 +309,11 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     const uint32_t bar_base = smem_base + STAGES * S::STAGE_BYTES;   // full[STAGES], empty[STAGES]
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    // Column tiling (DESIGN.md 6.1 "ragged and narrow tiles"): tiles_wide tiles of BN columns first,
-    // then tiles_narrow tiles of narrow_w columns (launched last, so that the tail of the launch is
-    // made of short CTAs).  A tile with `ncols_tile` valid columns only computes its first
-    // ceil(ncols_tile / 8) 8-column MMA blocks; block nb belongs to warp column nb % WARPS_N, so the
-    // remaining work stays balanced over the warps and the tile's time is ~ ceil(nblk / WARPS_N).
-    int tile_m, tile_n, n0, ncols_tile;
-    {
-        const int wide_ctas = p.tiles_m * p.tiles_wide;
-        if ((int)blockIdx.x < wide_ctas) {
-            tile_coords<C::GROUP_N>(blockIdx.x, p.tiles_m, p.tiles_wide, tile_m, tile_n);
-            n0 = tile_n * BN;
-            ncols_tile = min(BN, p.n - n0);
-        } else {
-            tile_coords<C::GROUP_N>(blockIdx.x - wide_ctas, p.tiles_m, p.tiles_narrow, tile_m, tile_n);
-            n0 = p.tiles_wide * BN + tile_n * p.narrow_w;
-            ncols_tile = min(p.narrow_w, p.n - n0);
-        }
-    }
-    const int m0 = tile_m * BM;
-    const int nblk = (ncols_tile + 7) >> 3;
     const int KT = (int)((p.N + BK - 1) / BK);
+    const bool is_dp = (int)blockIdx.x < p.dp_tiles;
+    const int sk_g = (int)blockIdx.x - p.dp_tiles;
+    int s_cur = 0, s_end = 0;
+    if (!is_dp) { s_cur = p.sk_begin[sk_g]; s_end = p.sk_begin[sk_g + 1]; }
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -296,37 +323,69 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    // Programmatic dependent launch: the next step's CTAs may be dispatched as soon as every CTA of this
+    // launch has got here (they then run their prologue and first H loads while this launch drains).
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     if (warp >= kConsumerWarps) {
         // ------------------------------------------------------------ producer warpgroup
         // gives its registers to the consumers (setmaxnreg is per warpgroup); one lane issues TMA
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         if (warp == kConsumerWarps && lane == 0) {
-            for (int kt = 0; kt < KT; ++kt) {
-                const int s = kt % STAGES;
-                const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
-                if (kt >= STAGES) mbar_wait(empty, ((kt / STAGES) - 1) & 1);
-                const uint32_t sa = smem_base + s * S::STAGE_BYTES, sb = sa + S::A_BYTES;
-                mbar_expect_tx(full, S::STAGE_BYTES);
-                const int k0 = kt * BK;
-                if (!p.a_2d) {
-                    // A: view (16 doubles, k, m_group); one box {16, BK, BM / ROWS128}
-                    tma_load_3d(sa, &tmapA, full, 0, k0, m0 / C::ROWS128);
-                } else {
-                    // A: view (doubles along m, k); one box {16, BK} per 128-byte row group -- the same
-                    // shared-memory image, rows past M zero-filled (any M, e.g. the paper's odd sizes)
+            // H is never written, so its first tiles may be fetched before the previous launch (which
+            // produces this step's X) has finished; X loads and everything after wait for it.
+            bool dep_waited = false;
+            uint32_t it = 0;
+            Segment seg;
+            while (next_segment(p, KT, is_dp, s_cur, s_end, seg)) {
+                int tile_m, tile_n;
+                tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+                const int m0 = tile_m * BM, n0 = tile_n * p.bn_w;
+                auto load_A = [&](uint32_t slot, int kt) {
+                    const uint32_t full = bar_base + 8 * slot;
+                    const uint32_t sa = smem_base + slot * S::STAGE_BYTES;
+                    const int k0 = kt * BK;
+                    mbar_expect_tx(full, S::STAGE_BYTES);
+                    if (!p.a_2d) {
+                        // A: view (16 doubles, k, m_group); one box {16, BK, BM / ROWS128}
+                        tma_load_3d(sa, &tmapA, full, 0, k0, m0 / C::ROWS128);
+                    } else {
+                        // A: view (doubles along m, k); one box {16, BK} per 128-byte row group -- the same
+                        // shared-memory image, rows past M zero-filled (any M, e.g. the paper's odd sizes)
 #pragma unroll 4
-                    for (int gI = 0; gI < BM / C::ROWS128; ++gI)
-                        tma_load_2d(sa + gI * BK * 128, &tmapA, full, (m0 + gI * C::ROWS128) * (CPLX ? 2 : 1), k0);
-                }
-                // B: (doubles along k, column); boxes {16 doubles, BN}
-                if (CPLX) {
-                    tma_load_2d(sb, &tmapB, full, 2 * k0, p.col0 + n0);
-                    tma_load_2d(sb + BN * 128, &tmapB, full, 2 * k0 + 16, p.col0 + n0);
-                } else {
+                        for (int gI = 0; gI < BM / C::ROWS128; ++gI)
+                            tma_load_2d(sa + gI * BK * 128, &tmapA, full, (m0 + gI * C::ROWS128) * (CPLX ? 2 : 1), k0);
+                    }
+                };
+                auto load_B = [&](uint32_t slot, int kt) {
+                    const uint32_t full = bar_base + 8 * slot;
+                    const uint32_t sb = smem_base + slot * S::STAGE_BYTES + S::A_BYTES;
+                    const int k0 = kt * BK;
+                    // B: (doubles along k, column); boxes {16 doubles, BN}
+                    if (CPLX) {
+                        tma_load_2d(sb, &tmapB, full, 2 * k0, p.col0 + n0);
+                        tma_load_2d(sb + BN * 128, &tmapB, full, 2 * k0 + 16, p.col0 + n0);
+                    } else {
 #pragma unroll
-                    for (int kq = 0; kq < BK / 16; ++kq)
-                        tma_load_2d(sb + kq * BN * 128, &tmapB, full, k0 + 16 * kq, p.col0 + n0);
+                        for (int kq = 0; kq < BK / 16; ++kq)
+                            tma_load_2d(sb + kq * BN * 128, &tmapB, full, k0 + 16 * kq, p.col0 + n0);
+                    }
+                };
+                int kt = seg.k0;
+                if (!dep_waited) {
+                    const int pre = min(STAGES, seg.k1 - seg.k0);       // ring is empty: no empty-wait needed
+                    for (int i = 0; i < pre; ++i) load_A(i, kt + i);
+                    asm volatile("griddepcontrol.wait;" ::: "memory");
+                    for (int i = 0; i < pre; ++i) load_B(i, kt + i);
+                    dep_waited = true;
+                    kt += pre;
+                    it += pre;
+                }
+                for (; kt < seg.k1; ++kt, ++it) {
+                    const uint32_t slot = it % STAGES;
+                    if (it >= (uint32_t)STAGES) mbar_wait(bar_base + 8 * (STAGES + slot), ((it / STAGES) - 1) & 1);
+                    load_A(slot, kt);
+                    load_B(slot, kt);
                 }
             }
         }
@@ -335,60 +394,140 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     // ---------------------------------------------------------------- consumer warps
     asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");     // X, Y and the stream-K scratch belong to the previous launch until here
     const int g = lane >> 2, t = lane & 3;
     constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
     static_assert(WARPS_N * C::WN == BN, "warp grid must cover the CTA tile");
+    static_assert((CPLX ? 2 : 1) * MB * NB * 16 * kConsumerThreads == kPartBytes, "partial tile size");
     const int wm = warp % C::WARPS_M, wn = warp / C::WARPS_M;
-    const int jmax = (nblk - wn + WARPS_N - 1) / WARPS_N;    // this warp owns blocks nb = j * WARPS_N + wn, j < jmax
-
-    double acc[CPLX ? 2 : 1][MB][NB][2];
-#pragma unroll
-    for (int q = 0; q < (CPLX ? 2 : 1); ++q)
-#pragma unroll
-        for (int i = 0; i < MB; ++i)
-#pragma unroll
-            for (int j = 0; j < NB; ++j) acc[q][i][j][0] = acc[q][i][j][1] = 0.0;
-
-    if (jmax == NB) mainloop<CPLX, true>(acc, smem, bar_base, KT, lane, warp, jmax);
-    else mainloop<CPLX, false>(acc, smem, bar_base, KT, lane, warp, jmax);
-
-    // ---------------------------------------------------------------- fused epilogue
-    // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
-    const double alpha = p.alpha, beta = p.beta;
+    const int tid = threadIdx.x;                           // 0 .. kConsumerThreads-1 here
     constexpr int NC = CPLX ? 2 : 1;
+
+    uint32_t it = 0;
+    Segment seg;
+    while (next_segment(p, KT, is_dp, s_cur, s_end, seg)) {
+        // Column tiling: tiles of bn_w columns; a tile with `ncols_tile` valid columns only
+        // computes its first ceil(ncols_tile / 8) 8-column MMA blocks; block nb belongs to warp column
+        // nb % WARPS_N, so the work stays balanced over the warps and the tile's time is ~ ceil(nblk / WARPS_N).
+        int tile_m, tile_n;
+        tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+        const int m0 = tile_m * BM, n0 = tile_n * p.bn_w;
+        const int ncols_tile = min(p.bn_w, p.n - n0);
+        const int nblk = (ncols_tile + 7) >> 3;
+        const int jmax = (nblk - wn + WARPS_N - 1) / WARPS_N;    // this warp owns blocks nb = j * WARPS_N + wn, j < jmax
+
+        double acc[NC][MB][NB][2];
 #pragma unroll
-    for (int j = 0; j < NB; ++j) {
+        for (int q = 0; q < NC; ++q)
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const int cl = (j * WARPS_N + wn) * 8 + 2 * t + e;     // column inside the tile
-            if (cl >= ncols_tile) continue;
-            const int col = n0 + cl;
-            const double c = p.c_col ? p.c_col[col] : p.c;
+            for (int i = 0; i < MB; ++i)
 #pragma unroll
-            for (int i = 0; i < MB; ++i) {
-                int row;
-                if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
-                else row = m0 + wm * C::WM + (i >> 1) * 16 + 2 * g + (i & 1);
-                if (row >= p.M) continue;
-                const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
-                if (CPLX) {
-                    const double2 x = *reinterpret_cast<const double2 *>(p.X + off);
-                    double2 y;
-                    y.x = alpha * (acc[0][i][j][e] - c * x.x);
-                    y.y = alpha * (acc[NC - 1][i][j][e] - c * x.y);
-                    if (p.use_beta) {
-                        const double2 o = *reinterpret_cast<const double2 *>(p.Y + off);
-                        y.x = fma(beta, o.x, y.x);
-                        y.y = fma(beta, o.y, y.y);
+                for (int j = 0; j < NB; ++j) acc[q][i][j][0] = acc[q][i][j][1] = 0.0;
+
+        const int len = seg.k1 - seg.k0;
+        if (jmax == NB) mainloop<CPLX, true>(acc, smem, bar_base, it, len, lane, warp, jmax);
+        else mainloop<CPLX, false>(acc, smem, bar_base, it, len, lane, warp, jmax);
+        it += (uint32_t)len;
+
+        if (seg.k1 < KT) {
+            // ---- stream-K: this CTA stops inside the tile: park the partial sums, raise the flag
+            unsigned char *part = p.sk_part + (size_t)sk_g * kPartBytes;
+#pragma unroll
+            for (int q = 0; q < NC; ++q)
+#pragma unroll
+                for (int i = 0; i < MB; ++i)
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        if (j >= jmax) break;
+                        const int pr = (q * MB + i) * NB + j;
+                        *reinterpret_cast<double2 *>(part + ((size_t)pr * kConsumerThreads + tid) * 16) =
+                            make_double2(acc[q][i][j][0], acc[q][i][j][1]);
                     }
-                    *reinterpret_cast<double2 *>(p.Y + off) = y;
-                    for (int q = 0; q < p.npeers; ++q)      // fused all-gather: push the row block over NVLink
-                        *reinterpret_cast<double2 *>(p.peer_Y[q] + off) = y;
-                } else {
-                    double y = alpha * (acc[0][i][j][e] - c * p.X[off]);
-                    if (p.use_beta) y = fma(beta, p.Y[off], y);
-                    p.Y[off] = y;
-                    for (int q = 0; q < p.npeers; ++q) p.peer_Y[q][off] = y;
+            __threadfence();
+            asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+            if (tid == 0)
+                asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.sk_flag + sk_g), "r"(p.epoch) : "memory");
+            continue;
+        }
+        if (seg.k0 > 0) {
+            // ---- stream-K: this CTA finishes a tile that lower-numbered CTAs started: add their partials
+            const int tile_first = (seg.tile - p.dp_tiles) * KT;       // slab index of the tile's k-slab 0
+            for (int c = sk_g - 1; c >= 0; --c) {
+                const int cb = p.sk_begin[c], ce = p.sk_begin[c + 1];
+                if (ce > cb) {                                         // (an empty CTA parks nothing)
+                    if (tid == 0) {
+                        uint32_t v;
+                        unsigned long long t0 = 0;
+                        for (uint32_t spins = 0;; ++spins) {
+                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p.sk_flag + c) : "memory");
+                            if (v == p.epoch) break;
+                            if ((spins & 1023u) == 1023u) {            // a lost partial must not pass silently:
+                                unsigned long long now;                // trap after 20 s without the flag
+                                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                                if (t0 == 0) t0 = now;
+                                else if (now - t0 > 20000000000ull) __trap();
+                            }
+                            __nanosleep(32);
+                        }
+                    }
+                    __syncwarp();
+                    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+                    const unsigned char *part = p.sk_part + (size_t)c * kPartBytes;
+#pragma unroll
+                    for (int q = 0; q < NC; ++q)
+#pragma unroll
+                        for (int i = 0; i < MB; ++i)
+#pragma unroll
+                            for (int j = 0; j < NB; ++j) {
+                                if (j >= jmax) break;
+                                const int pr = (q * MB + i) * NB + j;
+                                const double2 v = __ldcg(reinterpret_cast<const double2 *>(
+                                    part + ((size_t)pr * kConsumerThreads + tid) * 16));
+                                acc[q][i][j][0] += v.x;
+                                acc[q][i][j][1] += v.y;
+                            }
+                }
+                if (cb <= tile_first) break;                           // CTA c held the tile's first slab
+            }
+        }
+
+        // ---------------------------------------------------------------- fused epilogue
+        // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
+        const double alpha = p.alpha, beta = p.beta;
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int cl = (j * WARPS_N + wn) * 8 + 2 * t + e;     // column inside the tile
+                if (cl >= ncols_tile) continue;
+                const int col = n0 + cl;
+                const double c = p.c_col ? p.c_col[col] : p.c;
+#pragma unroll
+                for (int i = 0; i < MB; ++i) {
+                    int row;
+                    if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
+                    else row = m0 + wm * C::WM + (i >> 1) * 16 + 2 * g + (i & 1);
+                    if (row >= p.M) continue;
+                    const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
+                    if (CPLX) {
+                        const double2 x = *reinterpret_cast<const double2 *>(p.X + off);
+                        double2 y;
+                        y.x = alpha * (acc[0][i][j][e] - c * x.x);
+                        y.y = alpha * (acc[NC - 1][i][j][e] - c * x.y);
+                        if (p.use_beta) {
+                            const double2 o = *reinterpret_cast<const double2 *>(p.Y + off);
+                            y.x = fma(beta, o.x, y.x);
+                            y.y = fma(beta, o.y, y.y);
+                        }
+                        *reinterpret_cast<double2 *>(p.Y + off) = y;
+                        for (int q = 0; q < p.npeers; ++q)      // fused all-gather: push the row block over NVLink
+                            *reinterpret_cast<double2 *>(p.peer_Y[q] + off) = y;
+                    } else {
+                        double y = alpha * (acc[0][i][j][e] - c * p.X[off]);
+                        if (p.use_beta) y = fma(beta, p.Y[off], y);
+                        p.Y[off] = y;
+                        for (int q = 0; q < p.npeers; ++q) p.peer_Y[q][off] = y;
+                    }
                 }
             }
         }
@@ -415,10 +554,13 @@ EncodeTiledFn get_encode_fn() {
 }
 
 int sm_count() {
+    static int cached = 0;                  // one device kind per process is assumed for the plan heuristics
+    if (cached > 0) return cached;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0)
-        sms = 148;
+        return 148;
+    cached = sms;
     return sms;
 }
 
@@ -462,72 +604,119 @@ cudaError_t encode_maps(DmmaPlan *plan) {
     return cudaSuccess;
 }
 
-// Time of one launch in units of a "quarter" tile (8 * WARPS_N columns x BM rows over all of k) on `sms`
-// SMs, one CTA per SM, CTAs dispatched in blockIdx order to the SM that frees first: `wide` CTAs of
-// `wide_cost` quarters, then `narrow` CTAs of `narrow_cost`.  SM loads are kept as (load, count) levels.
-struct Level { double load; int count; };
-void assign(std::vector<Level> &lv, int64_t T, double cost) {
-    while (T > 0) {
-        if (lv.size() == 1 && T >= lv[0].count) {          // whole rounds at once
-            const int64_t rounds = T / lv[0].count;
-            lv[0].load += (double)rounds * cost;
-            T -= rounds * lv[0].count;
-            continue;
-        }
-        const Level lo = lv.front();                          // levels are sorted by ascending load
-        const int m = (int)std::min<int64_t>(lo.count, T);
-        lv.front().count -= m;
-        if (lv.front().count == 0) lv.erase(lv.begin());
-        const double nl = lo.load + cost;
-        size_t i = 0;
-        while (i < lv.size() && lv[i].load < nl - 1e-9) ++i;
-        if (i < lv.size() && std::fabs(lv[i].load - nl) <= 1e-9) lv[i].count += m;
-        else lv.insert(lv.begin() + i, Level{nl, m});
-        T -= m;
-    }
-}
-double makespan(int sms, int64_t wide, double wide_cost, int64_t narrow, double narrow_cost) {
-    std::vector<Level> lv{Level{0.0, sms}};
-    assign(lv, wide, wide_cost);
-    assign(lv, narrow, narrow_cost);
-    return lv.back().load;
-}
-
-// Chooses the column tiling of one launch: `wide` tiles of BN columns, then tiles of `narrow_w` columns
-// (a multiple of the quarter width Q = 8 * WARPS_N) over the rest, minimising the modelled makespan.
+// ---------------------------------------------------------------- the launch plan (host, no CUDA call)
+// Cost unit: one "quarter slab" = the MMAs of one k-slab on 8 * WARPS_N columns x BM rows; a tile with v valid
+// columns costs ceil(ceil(v / 8) / WARPS_N) quarters per slab (measured: DESIGN.md 6.1).
 template <bool CPLX>
-void choose_tiling(int64_t n, int tiles_m, int sms, int &tiles_wide, int &tiles_narrow, int &narrow_w) {
+void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan &pl) {
     using C = Cfg<CPLX>;
-    constexpr int Q = 8 * (kConsumerWarps / C::WARPS_M);      // columns per quarter tile
+    constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
+    constexpr int Q = 8 * WARPS_N;                            // columns per quarter tile
     constexpr int QPT = C::BN / Q;                            // quarters per full tile (4)
-    constexpr double kNarrowOverhead = 0.06;                  // per-CTA cost of a narrow tile beyond its quarters
-    const int full_tiles = (int)(n / C::BN);
-    double best = 1e300;
-    tiles_wide = full_tiles; tiles_narrow = 0; narrow_w = C::BN;
-    const int backs[4] = {0, 1, 2, full_tiles};                         // full tiles handed to the narrow region
-    for (int bi = 0; bi < 4; ++bi) {
-        const int back = backs[bi];
-        if (back > full_tiles || (bi == 3 && back <= 2)) continue;
-        const int wide = full_tiles - back;
-        const int64_t rest = n - (int64_t)wide * C::BN;
-        if (rest == 0) {
-            const double t = makespan(sms, (int64_t)wide * tiles_m, QPT, 0, 0.0);
-            if (t < best) { best = t; tiles_wide = wide; tiles_narrow = 0; narrow_w = C::BN; }
-            continue;
-        }
-        for (int wq = 1; wq <= QPT; ++wq) {
-            const int w = wq * Q;
-            const int64_t nt = (rest + w - 1) / w;
-            // cost of the narrow tiles: all but the last have wq quarters; model the last one the same
-            const double t = makespan(sms, (int64_t)wide * tiles_m, QPT, nt * tiles_m, wq + kNarrowOverhead);
-            // total work also matters when the launch is shorter than one wave: prefer fewer, wider tiles on ties
-            if (t < best - 1e-9) { best = t; tiles_wide = wide; tiles_narrow = (int)nt; narrow_w = w; }
+    constexpr int kMinWork = 4;                               // quarter slabs a stream-K CTA should at least get
+    const int KT = (int)((N + C::BK - 1) / C::BK);
+    const int tiles_m = (int)((M + C::BM - 1) / C::BM);
+    sms = std::max(1, std::min(sms, kMaxSkCtas));
+    // Column tile width: the full BN unless that leaves so few tiles that a tile would be split among
+    // more than ~6 stream-K CTAs (its finisher adds their partial tiles one after the other); then narrower.
+    int w = C::BN;
+    if (allow_sk) {
+        const int cand[3] = {C::BN, 2 * Q, Q};
+        for (int ci = 0; ci < 3; ++ci) {
+            w = cand[ci];
+            const int64_t T = (int64_t)tiles_m * ((n + w - 1) / w);
+            if (T * 6 >= sms) break;
         }
     }
+    const int tiles_n = (int)((n + w - 1) / w);
+    const int64_t T = (int64_t)tiles_m * tiles_n;
+    auto quarters_of_col_tile = [&](int tn) {
+        const int v = (int)std::min<int64_t>(w, n - (int64_t)tn * w);
+        const int nblk = (v + 7) / 8;
+        return (nblk + WARPS_N - 1) / WARPS_N;
+    };
+    const int q_full = quarters_of_col_tile(0), q_last = quarters_of_col_tile(tiles_n - 1);
+    auto quarters_of_tile = [&](int64_t t) {
+        int tm, tn;
+        tile_coords<C::GROUP_N>((int)t, tiles_m, tiles_n, tm, tn);
+        return tn == tiles_n - 1 ? q_last : q_full;
+    };
+    pl.KT = KT; pl.tiles_m = tiles_m; pl.tiles_n = tiles_n; pl.bn_w = w;
+    pl.dp_tiles = (int)T; pl.sk_ctas = 0; pl.sk_begin[0] = 0;
+    (void)QPT;
+    if (!allow_sk || T <= 0) return;
+
+    // Data-parallel region: whole waves, all but the last one-to-two waves' worth of tiles.
+    int64_t D = 0;
+    if (T >= 2 * (int64_t)sms) D = (T / sms - 1) * sms;
+    // SM free times after the data-parallel region (list scheduling in blockIdx order), ascending: the g-th
+    // stream-K CTA is the (D + g)-th CTA of the grid and starts on the g-th SM to become free.
+    std::vector<double> free_at((size_t)sms, 0.0);
+    if (D > 0) {
+        if (q_last == q_full) {
+            std::fill(free_at.begin(), free_at.end(), (double)(D / sms) * q_full * KT);
+        } else {
+            std::priority_queue<double, std::vector<double>, std::greater<double>> heap;
+            for (int i = 0; i < sms; ++i) heap.push(0.0);
+            for (int64_t t = 0; t < D; ++t) {
+                const double f = heap.top();
+                heap.pop();
+                heap.push(f + (double)quarters_of_tile(t) * KT);
+            }
+            for (int i = 0; i < sms; ++i) { free_at[(size_t)i] = heap.top(); heap.pop(); }
+        }
+    }
+    // Stream-K region: tiles [D, T); work in quarter slabs.
+    double work = 0.0;
+    for (int64_t t = D; t < T; ++t) work += (double)quarters_of_tile(t) * KT;
+    int G = sms;
+    if (work < (double)G * kMinWork) G = (int)std::max(1.0, work / kMinWork);
+    const int64_t R = T - D;
+    if (R < G && (int64_t)KT * q_full < 32 * (int64_t)(G / R)) {
+        // tiny launch: align the split with the tile boundaries (every CTA inside ONE tile)
+        G = (int)(R * (G / R));
+    }
+    if (G <= 1) return;                                        // too little work to split: one CTA per tile
+    if (D == 0 && R == G && q_last == q_full) return;          // one whole tile per CTA already: nothing to balance
+    // Water-filling: finish time F with sum_g max(0, F - free_at[g]) = work.
+    double F = 0.0;
+    {
+        double acc_f = 0.0;
+        int used = 0;
+        for (int gI = 0; gI < G; ++gI) {          // free_at ascending: try using CTAs 0..gI
+            acc_f += free_at[(size_t)gI];
+            used = gI + 1;
+            F = (work + acc_f) / used;
+            if (gI + 1 == G || F <= free_at[(size_t)gI + 1]) break;
+        }
+        (void)used;
+    }
+    pl.dp_tiles = (int)D;
+    pl.sk_ctas = G;
+    // Boundaries: walk the region's tiles, cutting where the cumulative cost reaches each CTA's share.
+    const int64_t total_slabs = R * KT;
+    double target = 0.0, cum = 0.0;            // cost before the current tile
+    int64_t t = D;
+    int qt = quarters_of_tile(t);
+    pl.sk_begin[0] = 0;
+    for (int gI = 0; gI < G; ++gI) {
+        target += std::max(0.0, F - free_at[(size_t)gI]);
+        // advance to the tile containing `target`
+        while (t < T - 1 && cum + (double)qt * KT <= target) {
+            cum += (double)qt * KT;
+            ++t;
+            qt = quarters_of_tile(t);
+        }
+        int64_t slab = (t - D) * KT + (int64_t)std::llround((target - cum) / qt);
+        slab = std::max<int64_t>(slab, pl.sk_begin[gI]);
+        slab = std::min<int64_t>(slab, total_slabs);
+        pl.sk_begin[gI + 1] = (int)slab;
+    }
+    pl.sk_begin[G] = (int)total_slabs;
 }
 
 template <bool CPLX>
-cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
+cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
                    cudaStream_t stream, const double *c_col) {
     using C = Cfg<CPLX>;
     static std::once_flag once;
@@ -539,6 +728,30 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
     if (attr_err != cudaSuccess) return attr_err;
     const int64_t n = plan->ncols - s;
     if (n <= 0) return cudaSuccess;
+
+    // The plan only depends on the active width: reuse it across the steps of one filter call.
+    if (plan->step_plan_n != n) {
+        try {
+            make_plan<CPLX>(plan->M, plan->N, n, sm_count(), true, plan->step_plan);
+        } catch (const std::exception &) {
+            return cudaErrorMemoryAllocation;
+        }
+        plan->step_plan_n = n;
+    }
+    const StepPlan &pl = plan->step_plan;
+
+    // Stream-K scratch: the caller's (chase_filter_ws: part of the workspace), else stream-ordered memory.
+    unsigned char *scratch = (unsigned char *)plan->sk_scratch;
+    bool own_scratch = false;
+    cudaError_t e;
+    if (pl.sk_ctas > 0 && !scratch) {
+        if ((e = cudaMallocAsync((void **)&scratch, dmma_sk_scratch_bytes(), stream)) != cudaSuccess) return e;
+        own_scratch = true;
+    }
+    if (pl.sk_ctas > 0 && (own_scratch || plan->sk_epoch == 0)) {       // flags start at 0, epochs at 1
+        if ((e = cudaMemsetAsync(scratch, 0, kSkFlagBytes, stream)) != cudaSuccess) return e;
+    }
+
     StepParams p;
     const size_t col_doubles = (size_t)plan->N * (CPLX ? 2 : 1);
     p.X = (const double *)plan->buf[src] + (size_t)s * col_doubles;
@@ -552,28 +765,47 @@ cudaError_t launch(const DmmaPlan *plan, int src, int64_t s, double alpha, doubl
         p.peer_Y[q] = (double *)plan->peer_buf[src ^ 1][q] + (size_t)s * col_doubles;
     p.n = (int)n;
     p.col0 = (int)s;
-    p.tiles_m = (int)((plan->M + C::BM - 1) / C::BM);
-    choose_tiling<CPLX>(n, p.tiles_m, sm_count(), p.tiles_wide, p.tiles_narrow, p.narrow_w);
+    p.tiles_m = pl.tiles_m;
+    p.tiles_n = pl.tiles_n;
+    p.bn_w = pl.bn_w;
+    p.dp_tiles = pl.dp_tiles;
+    p.sk_ctas = pl.sk_ctas;
+    p.epoch = own_scratch ? 1u : ++plan->sk_epoch;
+    p.sk_flag = (uint32_t *)scratch;
+    p.sk_part = scratch ? scratch + kSkFlagBytes : nullptr;
     p.alpha = alpha;
     p.beta = beta;
     p.c = c;
     p.c_col = c_col;
     p.use_beta = use_beta;
+    std::memcpy(p.sk_begin, pl.sk_begin, sizeof(int) * (size_t)(pl.sk_ctas + 1));
     const CUtensorMap *mA = (const CUtensorMap *)plan->tmap_H;
     const CUtensorMap *mB = (const CUtensorMap *)plan->tmap_B[src];
-    step_dmma_kernel<CPLX><<<(unsigned)(p.tiles_m * (p.tiles_wide + p.tiles_narrow)), kThreads, Smem<CPLX>::TOTAL, stream>>>(*mA, *mB, p);
+
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(pl.dp_tiles + pl.sk_ctas));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Smem<CPLX>::TOTAL;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, step_dmma_kernel<CPLX>, *mA, *mB, p);
     count_launch();
-    return cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (own_scratch) return cudaFreeAsync(scratch, stream);
+    return cudaSuccess;
 }
 
 }  // namespace
 
-void dmma_plan_tiling(int64_t N, int64_t n, chase_dtype_t dtype, int sms, int32_t out[4]) {
-    int tw = 0, tn = 0, nw = 0;
-    const int tiles_m = (int)((N + 127) / 128);
-    if (dtype == CHASE_C128) choose_tiling<true>(n, tiles_m, sms, tw, tn, nw);
-    else choose_tiling<false>(n, tiles_m, sms, tw, tn, nw);
-    out[0] = tiles_m; out[1] = tw; out[2] = tn; out[3] = nw;
+size_t dmma_sk_scratch_bytes() { return kSkFlagBytes + (size_t)kMaxSkCtas * kPartBytes; }
+
+void dmma_step_plan(int64_t N, int64_t n, chase_dtype_t dtype, int sms, StepPlan *out) {
+    if (dtype == CHASE_C128) make_plan<true>(N, N, n, sms, true, *out);
+    else make_plan<false>(N, N, n, sms, true, *out);
 }
 
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
@@ -583,6 +815,23 @@ bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     return false;
 }
 
+static void plan_common(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N, int64_t row0, int64_t nrows,
+                        int64_t ldh, void *V, void *W, int64_t ncols) {
+    plan->dtype = dtype;
+    plan->N = N;
+    plan->M = nrows;
+    plan->ldh = ldh;
+    plan->row0 = row0;
+    plan->npeers = 0;
+    plan->ncols = ncols;
+    plan->H = H;
+    plan->buf[0] = V;
+    plan->buf[1] = W;
+    plan->sk_scratch = nullptr;
+    plan->sk_epoch = 0;
+    plan->step_plan_n = -1;
+}
+
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N, void *V, void *W,
                              int64_t ncols) {
     return dmma_plan_create_rows(plan, dtype, H, N, 0, N, V, W, ncols);
@@ -590,36 +839,18 @@ cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H,
 
 cudaError_t dmma_plan_create_rows(DmmaPlan *plan, chase_dtype_t dtype, const void *H_loc, int64_t N, int64_t row0,
                                   int64_t nrows, void *V, void *W, int64_t ncols) {
-    plan->dtype = dtype;
-    plan->N = N;
-    plan->M = nrows;
-    plan->ldh = nrows;
-    plan->row0 = row0;
-    plan->npeers = 0;
-    plan->ncols = ncols;
-    plan->H = H_loc;
-    plan->buf[0] = V;
-    plan->buf[1] = W;
+    plan_common(plan, dtype, H_loc, N, row0, nrows, nrows, V, W, ncols);
     return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);
 }
 
 cudaError_t dmma_plan_create_panel(DmmaPlan *plan, chase_dtype_t dtype, const void *H_full, int64_t N, int64_t row0,
                                    int64_t nrows, void *V, void *W, int64_t ncols) {
     const size_t esz = dtype == CHASE_C128 ? 16 : 8;
-    plan->dtype = dtype;
-    plan->N = N;
-    plan->M = nrows;
-    plan->ldh = N;
-    plan->row0 = row0;
-    plan->npeers = 0;
-    plan->ncols = ncols;
-    plan->H = (const char *)H_full + (size_t)row0 * esz;
-    plan->buf[0] = V;
-    plan->buf[1] = W;
+    plan_common(plan, dtype, (const char *)H_full + (size_t)row0 * esz, N, row0, nrows, N, V, W, ncols);
     return dtype == CHASE_C128 ? encode_maps<true>(plan) : encode_maps<false>(plan);
 }
 
-cudaError_t dmma_launch_step(const DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c,
+cudaError_t dmma_launch_step(DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c,
                              int use_beta, cudaStream_t stream, const double *c_col) {
     return plan->dtype == CHASE_C128 ? launch<true>(plan, src, s, alpha, beta, c, use_beta, stream, c_col)
                                      : launch<false>(plan, src, s, alpha, beta, c, use_beta, stream, c_col);

@@ -52,3 +52,34 @@ def test_spectral_estimates_end_to_end_cfg2_shape():
     assert lam[-1] <= b_sup
     assert lam[0] <= mu1 + 1e-12 and mu1 < mune < b_sup
     assert abs(mune - lam[ne - 1]) <= 0.3
+
+
+@pytest.mark.parametrize("dtype,N", [(torch.complex128, 520), (torch.float64, 1040), (torch.complex64, 768)])
+def test_ritz_vectors_match_oracle_and_land_in_the_chosen_columns(dtype, N):
+    """Alg. 6 l.13: Ritz vectors of run 1 below mu_ne, interspersed into every other column of V^; the
+    other columns of V^ stay untouched; values and vectors equal the oracle's (unique sign)."""
+    k, nruns = 16, 3
+    w = W.make_config(2, N=N, ncols=nruns, dtype=dtype)
+    H, V0 = _dev(w.H), _dev(w.V0)
+    ws = torch.empty(pkg.chase_lanczos_workspace_bytes(N, nruns, k, dtype), dtype=torch.uint8, device="cuda:0")
+    alpha, beta = pkg.chase_lanczos(H, V0, k, workspace=ws)
+    mu_ne = -0.5
+    Vhat0 = W.gaussian_colmajor(N, 2 * k, dtype, seed=99)
+    Vhat = _dev(Vhat0)
+    dst = list(range(1, 2 * k, 2))                          # odd columns: interspersed with the random ones
+    vals = pkg.chase_lanczos_ritz_vectors(ws, N, dtype, alpha, beta, 1, mu_ne, Vhat, dst)
+    torch.cuda.synchronize()
+    Hn, Vn = w.H.numpy(), w.V0.numpy()
+    a_ref, b_ref, U_ref, _ = OL.lanczos(Hn, Vn[:, 1], k)
+    lam_ref, X_ref, _ = OL.ritz_vectors(U_ref, a_ref, b_ref, mu_ne)
+    assert 0 < len(lam_ref) < k and len(vals) == len(lam_ref)
+    tol = 1e-9 if dtype in (torch.complex128, torch.float64) else 2e-3
+    np.testing.assert_allclose(vals, lam_ref, atol=tol)
+    got = Vhat.cpu().numpy()
+    for i in range(len(vals)):
+        assert np.linalg.norm(got[:, dst[i]] - X_ref[:, i]) <= tol * 10, i
+    untouched = [c for c in range(2 * k) if c not in dst[: len(vals)]]
+    assert np.array_equal(got[:, untouched], Vhat0.numpy()[:, untouched])
+    # fewer target columns than Ritz vectors: the smallest Ritz values win
+    vals2 = pkg.chase_lanczos_ritz_vectors(ws, N, dtype, alpha, beta, 1, mu_ne, Vhat, dst[:2])
+    np.testing.assert_allclose(vals2, lam_ref[:2], atol=tol)

@@ -65,7 +65,7 @@ def test_schedule():
 
 
 def _raw_ws(H=0x1000, N=64, V=0x2000, ncols=4, degrees=(2, 2, 4, 4), a=-1.0, b=2.0, l1=-2.0,
-            dtype=3, ws=0x3000, ws_bytes=1 << 20):
+            dtype=3, ws=0x3000, ws_bytes=1 << 25):
     lib = pkg.load()
     deg = np.asarray(degrees, dtype=np.int32)
     return lib.chase_filter_ws(H, N, V, ncols, deg.ctypes.data if deg.size else None, a, b, l1, dtype,
@@ -96,7 +96,9 @@ def test_validation_rejects_before_any_launch():
 
 def test_workspace_bytes():
     import torch
-    assert pkg.chase_filter_workspace_bytes(40000, 2000, torch.complex128) == 40000 * 2000 * 16
+    sk = 1024 + 160 * 128 * 1024                            # FP64 tensor path: stream-K flags + partial tiles
+    assert pkg.chase_filter_workspace_bytes(40000, 2000, torch.complex128) == 40000 * 2000 * 16 + sk
+    assert pkg.chase_filter_workspace_bytes(60000, 3000, torch.complex64) == 60000 * 3000 * 8 + 256
     assert pkg.chase_filter_workspace_bytes(3, 1, torch.float32) == 256
     assert pkg.load().chase_filter_workspace_bytes(10, 10, 9) == 0
 
@@ -126,25 +128,76 @@ def test_product_does_not_import_oracle():
             assert "#include \"chase" not in src, f
 
 
-@pytest.mark.parametrize("dtype,bn,quarter", [(torch.complex128, 64, 16), (torch.float64, 128, 32)])
-def test_step_tiling_covers_every_column_once(dtype, bn, quarter):
-    """chase_filter_step_tiling: wide tiles then narrow tiles cover [0, n) exactly; the narrow width is a
-    multiple of the quarter width; never more narrow columns than needed (host model only, no CUDA)."""
-    for N in (512, 4096, 40000):
-        for n in list(range(1, 200)) + [255, 256, 257, 1400, 1867, 2000, 2999]:
+@pytest.mark.parametrize("dtype,bn,quarter,bk", [(torch.complex128, 64, 16, 16), (torch.float64, 128, 32, 32)])
+def test_step_plan_covers_every_tile_slab_exactly_once(dtype, bn, quarter, bk):
+    """chase_filter_step_plan (host model only, no CUDA): the column tiles cover [0, n) exactly; the
+    data-parallel tiles plus the stream-K ranges cover every k-slab of every tile exactly once; ranges
+    are contiguous and ascending (a CTA only ever waits on lower-numbered CTAs)."""
+    for N in (64, 512, 4096, 40000):
+        for n in list(range(1, 70)) + [96, 127, 128, 129, 255, 256, 257, 1400, 1867, 2000, 2999]:
             for sms in (148, 132):
-                tm, tw, tn, nw = pkg.chase_filter_step_tiling(N, n, dtype, sms)
-                assert tm == -(-N // 128)
-                assert 0 <= tw * bn <= n
-                rest = n - tw * bn
-                assert nw % quarter == 0 and quarter <= nw <= bn
-                assert tn == -(-rest // nw), (N, n, tw, tn, nw)
+                pl = pkg.chase_filter_step_plan(N, n, dtype, sms)
+                w, tm, tn = pl["tile_width"], pl["tiles_m"], pl["tiles_n"]
+                assert tm == -(-N // 128) and pl["slabs_per_tile"] == -(-N // bk)
+                assert w % quarter == 0 and quarter <= w <= bn
+                assert tn == -(-n // w), (N, n, w, tn)
+                T, D, G, KT = tm * tn, pl["dp_tiles"], pl["sk_ctas"], pl["slabs_per_tile"]
+                assert 0 <= D <= T and 0 <= G <= min(sms, 160)
+                skb = pl["sk_begin"]
+                if G == 0:
+                    assert D == T
+                    continue
+                assert D % sms == 0                                # the data-parallel part is whole waves
+                assert len(skb) == G + 1 and skb[0] == 0 and skb[-1] == (T - D) * KT
+                assert np.all(np.diff(skb) >= 0)
 
 
-def test_step_tiling_shortens_the_tail_of_the_metric_config():
-    """cfg 4 full width: 2000 = 31 x 64 + 16 columns; the ragged 16 columns must not cost a full tile."""
-    tm, tw, tn, nw = pkg.chase_filter_step_tiling(40000, 2000, torch.complex128, 148)
-    assert (tm, tw) == (313, 31) and tn * nw >= 16 and nw < 64
+def test_step_plan_balances_the_benchmark_configs():
+    """Modelled makespan (quarter-slab units, one CTA per SM, dispatch in blockIdx order) of the plan
+    vs the perfect split: cfg 1 (latency-bound: 16 tiles for 148 SMs), cfg 2 (128 tiles for 148 SMs),
+    cfg 4 full width (10016 tiles, ragged last column tile)."""
+    import heapq
+
+    def makespan(N, n, dtype, sms=148):
+        pl = pkg.chase_filter_step_plan(N, n, dtype, sms)
+        cplx = dtype == torch.complex128
+        warps_n, group_n = (2, 16) if cplx else (4, 12)
+        w, tm, tn, KT = pl["tile_width"], pl["tiles_m"], pl["tiles_n"], pl["slabs_per_tile"]
+
+        def quarters(t):                                          # cost of one slab of raster tile t
+            per_group = group_n * tm
+            grp = t // per_group
+            first = grp * group_n
+            gn = min(group_n, tn - first)
+            col = first + (t - grp * per_group) % gn
+            v = min(w, n - col * w)
+            return -(-(-(-v // 8)) // warps_n)
+
+        heap = [0.0] * sms
+        total = 0.0
+        for t in range(pl["dp_tiles"]):
+            f = heapq.heappop(heap)
+            heapq.heappush(heap, f + quarters(t) * KT)
+            total += quarters(t) * KT
+        end = max(heap) if pl["sk_ctas"] == 0 else 0.0
+        skb = pl["sk_begin"]
+        for g in range(pl["sk_ctas"]):
+            f = heapq.heappop(heap)
+            cost, s = 0.0, int(skb[g])
+            while s < skb[g + 1]:
+                t = pl["dp_tiles"] + s // KT
+                take = min(int(skb[g + 1]) - s, KT - s % KT)
+                cost += take * quarters(t)
+                s += take
+            total += cost
+            end = max(end, f + cost)
+        return end, total / sms
+
+    for N, n, dtype, slack in ((512, 60, torch.complex128, 1.10), (4096, 256, torch.complex128, 1.01),
+                               (4096, 37, torch.complex128, 1.03), (40000, 2000, torch.complex128, 1.002),
+                               (40000, 1867, torch.complex128, 1.002), (20000, 1400, torch.float64, 1.002)):
+        end, ideal = makespan(N, n, dtype)
+        assert end <= slack * ideal + 4, (N, n, end, ideal)
 
 
 def test_rows_and_lanczos_validation_rejects_before_any_launch():
@@ -211,6 +264,20 @@ def test_rows_and_lanczos_validation_rejects_before_any_launch():
     assert lanczos(ws=None) == -5
     assert lanczos(ws_bytes=1024) == -5
     assert lanczos(ws=0x7008) == -6
+
+    cnt = C.c_int64(-1)
+    dst = np.asarray([0, 1], dtype=np.int64)
+    def ritz_vecs(run=1, nruns=2, k=5, ws=0x7000, ws_bytes=1 << 24, vhat=Y, ncv=4, d=dst, mu=0.0):
+        return lib.chase_lanczos_ritz_vectors(ws, ws_bytes, 64, nruns, k, 3, run, al.ctypes.data, al.ctypes.data, mu,
+                                              vhat, ncv, d.ctypes.data, d.size, C.addressof(cnt), None, None)
+    assert ritz_vecs(run=2) == -1                          # run out of range
+    assert ritz_vecs(k=0) == -1
+    assert ritz_vecs(vhat=None) == -1
+    assert ritz_vecs(d=np.asarray([0, 4], dtype=np.int64)) == -1      # target column outside Vhat
+    assert ritz_vecs(mu=float("nan")) == -1
+    assert ritz_vecs(ws=None) == -5
+    assert ritz_vecs(ws_bytes=64) == -5
+    assert ritz_vecs(vhat=0x3008) == -6
     assert pkg.chase_filter_launch_count() == before
 
 

@@ -149,3 +149,40 @@ def test_L7_gue_estimates_are_sane():
     assert lam_true[-1] <= b_sup <= lam_true[-1] + runs[0][1][-1] + 1e-12   # loose by at most ||f_k|| (~1 for GUE)
     assert lam_true[0] - 1e-12 <= mu1 <= lam_true[0] + 0.1
     assert abs(mune - lam_true[nev_nex - 1]) <= 0.3
+
+
+def test_l8_ritz_vectors_residual_identity_and_orthonormality():
+    """Alg. 6 l.13.  Pins oracle.lanczos.ritz_vectors with what the mathematics fixes:
+    the classical Lanczos residual identity  ||A x_i - lam~_i x_i||_2 = beta_k |Z_{k,i}|  (from
+    A U = U T + f e_k^T, ||f|| = beta_k), orthonormality of the x_i, Rayleigh quotients x_i^H A x_i = lam~_i,
+    the selection lam~_i < mu_ne in ascending order, and -- for k = N, where the Krylov space is the whole
+    space -- that the Ritz pairs ARE the eigenpairs of A (eigh), up to the fixed sign."""
+    rng = np.random.default_rng(77)
+    N, k = 120, 14
+    G = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    A = (G + G.conj().T) / np.sqrt(2 * N)
+    v0 = rng.standard_normal(N) + 1j * rng.standard_normal(N)
+    alpha, beta, U, f = OL.lanczos(A, v0, k)
+    mu = 0.3
+    lam, X, zk = OL.ritz_vectors(U, alpha, beta, mu)
+    all_lam, _ = OL.ritz(alpha, beta)
+    assert len(lam) == int(np.sum(all_lam < mu)) and 0 < len(lam) < k
+    assert np.all(np.diff(lam) > 0) and np.all(lam < mu)
+    R = A @ X - X * lam[None, :]
+    np.testing.assert_allclose(np.linalg.norm(R, axis=0), beta[-1] * zk, rtol=1e-9, atol=1e-12)
+    np.testing.assert_allclose(X.conj().T @ X, np.eye(len(lam)), atol=1e-12)
+    np.testing.assert_allclose(np.real(np.einsum("ij,ij->j", X.conj(), A @ X)), lam, atol=1e-12)
+    # a wrong index (e.g. Z rows instead of columns) or a transposed operand breaks the identity above;
+    # the direction of the residual pins it further: R = f * Z_{k,i} exactly
+    Zk_signed = (X.conj().T @ U[:, -1:])[:, 0].conj()      # = Z_{k,i} since x_i = U z_i, U orthonormal
+    np.testing.assert_allclose(R, np.outer(f, Zk_signed), atol=1e-10)
+
+    # k = N: Ritz pairs = eigenpairs
+    N2 = 24
+    A2 = A[:N2, :N2]
+    alpha2, beta2, U2, _ = OL.lanczos(A2, v0[:N2], N2)
+    lam2, X2, _ = OL.ritz_vectors(U2, alpha2, beta2, np.inf)
+    w, Q = np.linalg.eigh(A2)
+    np.testing.assert_allclose(lam2, w, atol=1e-10)
+    overlap = np.abs(np.einsum("ij,ij->j", Q.conj(), X2))
+    np.testing.assert_allclose(overlap, 1.0, atol=1e-8)
