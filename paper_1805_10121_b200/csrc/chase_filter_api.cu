@@ -147,13 +147,19 @@ int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t nc
                            cudaStream_t stream, void *sk_scratch) {
     const int path = chase_filter_kernel_path(N, ncols, dtype);
     const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
-    // A few vectors: one streaming pass over H.  In FP64 the narrow-tile DMMA kernel is the faster
-    // streamer from 3 columns on (measured: c128, N = 40000, 5 columns: 4.1 vs 3.0 TB/s).
-    const bool fp64_tensor = path == 1 && ncols > 2;
+    // A few vectors: one streaming pass over H (roofline: HBM).  Measured at c128, N = 40000 on the bulk-copy
+    // streaming kernel: 7.2 TB/s (1-2 columns), 6.7 (5), 4.5 (8: FP64 FMA-bound) against 5.5 TB/s for the
+    // stream-K narrow-tile tensor kernel, which therefore takes FP64 blocks of 7 and 8 columns.
+    // CHASE_SKINNY_FP64=stream / dmma overrides (experiments).
+    const char *fp64_mode = std::getenv("CHASE_SKINNY_FP64");
+    bool fp64_tensor = path == 1 && ncols > 6;
+    if (path == 1 && fp64_mode && fp64_mode[0] == 's') fp64_tensor = false;
+    if (path == 1 && fp64_mode && fp64_mode[0] == 'd') fp64_tensor = true;
     if (ncols <= kSkinnyMaxCols && !fp64_tensor && !(force && force[0] == '1')) {
         StepArgs sa;
         sa.H = H; sa.X = X; sa.Y = Y; sa.N = N; sa.n = ncols;
         sa.alpha = alpha; sa.beta = beta; sa.c = c; sa.c_col = c_col; sa.use_beta = use_beta;
+        if (stream_supported(dtype, sa)) return (int)launch_step_stream(dtype, sa, stream);
         return (int)launch_step_skinny(dtype, sa, stream);
     }
     if (path == 1) {

@@ -30,6 +30,10 @@ cudaError_t launch_step_generic(chase_dtype_t dtype, const StepArgs &a, cudaStre
 // bound by one pass over H from HBM.  Uses that H is Hermitian.
 constexpr int kSkinnyMaxCols = 8;
 cudaError_t launch_step_skinny(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
+// Same operation through a ring of bulk copies (csrc/step_stream.cu): persistent CTAs, long sequential
+// DRAM bursts.  Needs 16-byte aligned H, X and columns (N * sizeof(element) % 16 == 0), N >= 64.
+bool stream_supported(chase_dtype_t dtype, const StepArgs &a);
+cudaError_t launch_step_stream(chase_dtype_t dtype, const StepArgs &a, cudaStream_t stream);
 
 // TMA + DMMA tensor kernels (CHASE_C128 with any N >= 16, CHASE_F64 with even N).
 // Work decomposition of one launch on `n` active columns (csrc/step_dmma.cu): tiles of

@@ -19,6 +19,7 @@ namespace chase {
 namespace {
 
 constexpr int kBlock = 256;
+constexpr int kRedBlock = 1024;   // the reductions run one block per (vector pair): wide blocks, 4 loads in flight per thread
 
 __device__ __forceinline__ double2 ld(const float *p, int64_t i)   { return make_double2((double)p[i], 0.0); }
 __device__ __forceinline__ double2 ld(const double *p, int64_t i)  { return make_double2(p[i], 0.0); }
@@ -29,9 +30,9 @@ __device__ __forceinline__ void st(double *p, int64_t i, double2 v)  { p[i] = v.
 __device__ __forceinline__ void st(float2 *p, int64_t i, double2 v)  { p[i] = make_float2((float)v.x, (float)v.y); }
 __device__ __forceinline__ void st(double2 *p, int64_t i, double2 v) { p[i] = v; }
 
-// Sum of a double2 over the block; result valid in thread 0.
+// Sum of a double2 over the block (any block size that is a multiple of 32, up to 1024); result valid in thread 0.
 __device__ __forceinline__ double2 block_sum(double2 v) {
-    __shared__ double2 part[kBlock / 32];
+    __shared__ double2 part[32];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         v.x += __shfl_down_sync(0xffffffffu, v.x, o);
@@ -40,7 +41,7 @@ __device__ __forceinline__ double2 block_sum(double2 v) {
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = v;
     __syncthreads();
     if (threadIdx.x < 32) {
-        v = threadIdx.x < kBlock / 32 ? part[threadIdx.x] : make_double2(0.0, 0.0);
+        v = threadIdx.x < (blockDim.x >> 5) ? part[threadIdx.x] : make_double2(0.0, 0.0);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             v.x += __shfl_down_sync(0xffffffffu, v.x, o);
@@ -53,18 +54,25 @@ __device__ __forceinline__ double2 block_sum(double2 v) {
 // h[i, c] = U_i[:, c]^H w[:, c]  for i = blockIdx.x <= j, run c = blockIdx.y.  U_i is block i of U
 // (each block N x nvec, column-major).  pass 0 also records alpha_j[c] = Re h[j, c].
 template <typename T>
-__global__ void __launch_bounds__(kBlock) lz_project(const T *__restrict__ U, const T *__restrict__ w, int64_t N,
-                                                     int nvec, int j, double2 *__restrict__ h,
-                                                     double *__restrict__ alpha, int k, int pass) {
+__global__ void __launch_bounds__(kRedBlock) lz_project(const T *__restrict__ U, const T *__restrict__ w, int64_t N,
+                                                        int nvec, int j, double2 *__restrict__ h,
+                                                        double *__restrict__ alpha, int k, int pass) {
     const int i = blockIdx.x, c = blockIdx.y;
     const T *u = U + ((int64_t)i * nvec + c) * N;
     const T *x = w + (int64_t)c * N;
-    double2 acc = make_double2(0.0, 0.0);
-    for (int64_t r = threadIdx.x; r < N; r += kBlock) {
-        const double2 a = ld(u, r), b = ld(x, r);
-        acc.x += a.x * b.x + a.y * b.y;          // conj(a) * b
-        acc.y += a.x * b.y - a.y * b.x;
+    double2 a4[4] = {};
+    for (int64_t r0 = threadIdx.x; r0 < N; r0 += 4 * kRedBlock) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int64_t r = r0 + (int64_t)q * kRedBlock;
+            if (r < N) {
+                const double2 a = ld(u, r), b = ld(x, r);
+                a4[q].x += a.x * b.x + a.y * b.y;          // conj(a) * b
+                a4[q].y += a.x * b.y - a.y * b.x;
+            }
+        }
     }
+    double2 acc = make_double2((a4[0].x + a4[1].x) + (a4[2].x + a4[3].x), (a4[0].y + a4[1].y) + (a4[2].y + a4[3].y));
     acc = block_sum(acc);
     if (threadIdx.x == 0) {
         h[(int64_t)i * nvec + c] = acc;
@@ -92,15 +100,22 @@ __global__ void __launch_bounds__(kBlock) lz_update(const T *__restrict__ U, T *
 
 // out[c * stride + idx] = || x[:, c] ||_2
 template <typename T>
-__global__ void __launch_bounds__(kBlock) lz_colnorm(const T *__restrict__ x, int64_t N, double *__restrict__ out,
-                                                     int stride, int idx) {
+__global__ void __launch_bounds__(kRedBlock) lz_colnorm(const T *__restrict__ x, int64_t N, double *__restrict__ out,
+                                                        int stride, int idx) {
     const int c = blockIdx.x;
     const T *p = x + (int64_t)c * N;
-    double2 acc = make_double2(0.0, 0.0);
-    for (int64_t r = threadIdx.x; r < N; r += kBlock) {
-        const double2 a = ld(p, r);
-        acc.x += a.x * a.x + a.y * a.y;
+    double a4[4] = {};
+    for (int64_t r0 = threadIdx.x; r0 < N; r0 += 4 * kRedBlock) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int64_t r = r0 + (int64_t)q * kRedBlock;
+            if (r < N) {
+                const double2 a = ld(p, r);
+                a4[q] += a.x * a.x + a.y * a.y;
+            }
+        }
     }
+    double2 acc = make_double2((a4[0] + a4[1]) + (a4[2] + a4[3]), 0.0);
     acc = block_sum(acc);
     if (threadIdx.x == 0) out[(int64_t)c * stride + idx] = sqrt(acc.x);
 }
@@ -126,7 +141,7 @@ cudaError_t run(const void *H, int64_t N, const void *V0, int nvec, int k, chase
     T *w = U + (size_t)k * N * nvec;                                  // N x nvec
     const dim3 grid_rows((unsigned)((N + kBlock - 1) / kBlock), (unsigned)nvec);
     // u_0 = v_0 / ||v_0||; the start norm is parked in beta[.., 0] and overwritten by step 0
-    lz_colnorm<T><<<nvec, kBlock, 0, stream>>>((const T *)V0, N, d_beta, k, 0);
+    lz_colnorm<T><<<nvec, kRedBlock, 0, stream>>>((const T *)V0, N, d_beta, k, 0);
     lz_scale<T><<<grid_rows, kBlock, 0, stream>>>((const T *)V0, U, N, d_beta, k, 0);
     count_launch(); count_launch();
     for (int j = 0; j < k; ++j) {
@@ -134,11 +149,11 @@ cudaError_t run(const void *H, int64_t N, const void *V0, int nvec, int k, chase
         int rc = launch_one_step(H, N, uj, w, nvec, 1.0, 0.0, 0.0, nullptr, 0, dtype, stream);   // w = A u_j, all runs
         if (rc != 0) return rc > 0 ? (cudaError_t)rc : cudaErrorInvalidValue;
         for (int pass = 0; pass < 2; ++pass) {
-            lz_project<T><<<dim3(j + 1, nvec), kBlock, 0, stream>>>(U, w, N, nvec, j, d_h, d_alpha, k, pass);
+            lz_project<T><<<dim3(j + 1, nvec), kRedBlock, 0, stream>>>(U, w, N, nvec, j, d_h, d_alpha, k, pass);
             lz_update<T><<<grid_rows, kBlock, 0, stream>>>(U, w, N, nvec, j, d_h);
             count_launch(); count_launch();
         }
-        lz_colnorm<T><<<nvec, kBlock, 0, stream>>>(w, N, d_beta, k, j);     // beta_j = ||w||; j = k-1: ||f_k||
+        lz_colnorm<T><<<nvec, kRedBlock, 0, stream>>>(w, N, d_beta, k, j);     // beta_j = ||w||; j = k-1: ||f_k||
         count_launch();
         if (j + 1 < k) {
             lz_scale<T><<<grid_rows, kBlock, 0, stream>>>(w, U + (size_t)(j + 1) * N * nvec, N, d_beta, k, j);

@@ -22,15 +22,17 @@
 // Work decomposition of one launch (DESIGN.md 6.1 "stream-K tail"): the first `dp_tiles` CTAs own one
 // whole output tile each (data-parallel, grouped raster); the last `sk_ctas` CTAs share the remaining
 // tiles' k-slabs in equal-TIME contiguous ranges (stream-K): a CTA whose range ends inside a tile
-// leaves its partial accumulators in the scratch buffer and raises a flag, the CTA that reaches the
-// tile's last slab adds the partials of the lower-numbered CTAs and runs the fused epilogue.  A CTA
-// only ever waits on CTAs with a smaller blockIdx, which were dispatched before it.
+// leaves its partial accumulators in the scratch buffer and raises a flag -- first thing, because it
+// walks its range from the top down --, the CTA that holds the tile's last slab adds the partials of
+// the lower-numbered CTAs and runs the fused epilogue.  A CTA only ever waits on CTAs with a smaller
+// blockIdx, which were dispatched before it and parked their partial at the start of their life.
 // Launched with programmatic stream serialisation: prologue and the first H loads of step k+1
 // overlap the tail of step k (griddepcontrol).
 #include <cuda.h>
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <exception>
 #include <functional>
@@ -275,21 +277,26 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
 struct Segment {
     int tile, k0, k1;
 };
-// Segment `idx` of this CTA (DP CTAs have exactly one); false when the CTA's work is exhausted.
-// `s` walks the CTA's slab range of the stream-K region.
-__device__ __forceinline__ bool next_segment(const StepParams &p, int KT, bool is_dp, int &s, int s_end, Segment &seg) {
+// Next segment of this CTA (DP CTAs have exactly one); false when the CTA's work is exhausted.
+// A stream-K CTA walks its slab range [s_begin, s_end) from the TOP DOWN: the head of the last tile it
+// touches comes first -- it is parked at once for the higher-numbered CTA that holds that tile's tail --
+// and the tail of the first tile comes last, when the partial sums of the lower-numbered CTAs that hold
+// its head have long been parked.  (Bottom-up, every CTA would wait for the END of its predecessor.)
+__device__ __forceinline__ bool next_segment(const StepParams &p, int KT, bool is_dp, int s_begin, int &s_end,
+                                             Segment &seg) {
     if (is_dp) {
-        if (s != 0) return false;
+        if (s_end != 0) return false;
         seg.tile = blockIdx.x; seg.k0 = 0; seg.k1 = KT;
-        s = 1;
+        s_end = 1;
         return true;
     }
-    if (s >= s_end) return false;
-    const int tr = s / KT;
+    if (s_end <= s_begin) return false;
+    const int tr = (s_end - 1) / KT;
+    const int tile_first = tr * KT;
     seg.tile = p.dp_tiles + tr;
-    seg.k0 = s - tr * KT;
-    seg.k1 = min(KT, seg.k0 + (s_end - s));
-    s += seg.k1 - seg.k0;
+    seg.k1 = s_end - tile_first;
+    seg.k0 = max(s_begin, tile_first) - tile_first;
+    s_end = tile_first + seg.k0;
     return true;
 }
 
@@ -312,8 +319,8 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     const int KT = (int)((p.N + BK - 1) / BK);
     const bool is_dp = (int)blockIdx.x < p.dp_tiles;
     const int sk_g = (int)blockIdx.x - p.dp_tiles;
-    int s_cur = 0, s_end = 0;
-    if (!is_dp) { s_cur = p.sk_begin[sk_g]; s_end = p.sk_begin[sk_g + 1]; }
+    int s_begin = 0, s_end = 0;
+    if (!is_dp) { s_begin = p.sk_begin[sk_g]; s_end = p.sk_begin[sk_g + 1]; }
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -337,7 +344,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
             bool dep_waited = false;
             uint32_t it = 0;
             Segment seg;
-            while (next_segment(p, KT, is_dp, s_cur, s_end, seg)) {
+            while (next_segment(p, KT, is_dp, s_begin, s_end, seg)) {
                 int tile_m, tile_n;
                 tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
                 const int m0 = tile_m * BM, n0 = tile_n * p.bn_w;
@@ -405,7 +412,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     uint32_t it = 0;
     Segment seg;
-    while (next_segment(p, KT, is_dp, s_cur, s_end, seg)) {
+    while (next_segment(p, KT, is_dp, s_begin, s_end, seg)) {
         // Column tiling: tiles of bn_w columns; a tile with `ncols_tile` valid columns only
         // computes its first ceil(ncols_tile / 8) 8-column MMA blocks; block nb belongs to warp column
         // nb % WARPS_N, so the work stays balanced over the warps and the tile's time is ~ ceil(nblk / WARPS_N).
@@ -450,28 +457,72 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
             continue;
         }
         if (seg.k0 > 0) {
-            // ---- stream-K: this CTA finishes a tile that lower-numbered CTAs started: add their partials
+            // ---- stream-K: this CTA finishes a tile that lower-numbered CTAs started: add their partials.
+            // Contributors are the CTAs [c_lo, sk_g) with a non-empty range (CTA c_lo holds the tile's slab 0).
             const int tile_first = (seg.tile - p.dp_tiles) * KT;       // slab index of the tile's k-slab 0
-            for (int c = sk_g - 1; c >= 0; --c) {
-                const int cb = p.sk_begin[c], ce = p.sk_begin[c + 1];
-                if (ce > cb) {                                         // (an empty CTA parks nothing)
-                    if (tid == 0) {
-                        uint32_t v;
-                        unsigned long long t0 = 0;
-                        for (uint32_t spins = 0;; ++spins) {
-                            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p.sk_flag + c) : "memory");
-                            if (v == p.epoch) break;
-                            if ((spins & 1023u) == 1023u) {            // a lost partial must not pass silently:
-                                unsigned long long now;                // trap after 20 s without the flag
-                                asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
-                                if (t0 == 0) t0 = now;
-                                else if (now - t0 > 20000000000ull) __trap();
-                            }
-                            __nanosleep(32);
+            int c_lo = sk_g;
+            while (c_lo > 0) {
+                --c_lo;
+                if (p.sk_begin[c_lo] <= tile_first) break;
+            }
+            // all flags at once: thread t polls contributor c_lo + t (at most kMaxSkCtas < kConsumerThreads of them)
+            {
+                const int c = c_lo + tid;
+                if (c < sk_g && p.sk_begin[c + 1] > p.sk_begin[c]) {
+                    uint32_t v;
+                    unsigned long long t0 = 0;
+                    for (uint32_t spins = 0;; ++spins) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p.sk_flag + c) : "memory");
+                        if (v == p.epoch) break;
+                        if ((spins & 1023u) == 1023u) {            // a lost partial must not pass silently:
+                            unsigned long long now;                // trap after 20 s without the flag
+                            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                            if (t0 == 0) t0 = now;
+                            else if (now - t0 > 20000000000ull) __trap();
                         }
+                        __nanosleep(32);
                     }
-                    __syncwarp();
-                    asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+                }
+                __syncwarp();
+                asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");
+            }
+            if (sk_g - c_lo >= 3) {
+                // many small partials (a tile split among many CTAs: tiny launches): keep the loads of four
+                // contributors in flight at a time, one 8-column block after the other
+#pragma unroll
+                for (int j = 0; j < NB; ++j) {
+                    if (j >= jmax) break;
+                    for (int c = c_lo; c < sk_g; c += 4) {
+                        double2 v[4][NC][MB];
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const int cc = c + u;
+                            const bool ok = cc < sk_g && p.sk_begin[cc + 1] > p.sk_begin[cc];
+                            const unsigned char *part = p.sk_part + (size_t)(ok ? cc : c) * kPartBytes;
+#pragma unroll
+                            for (int q = 0; q < NC; ++q)
+#pragma unroll
+                                for (int i = 0; i < MB; ++i) {
+                                    const int pr = (q * MB + i) * NB + j;
+                                    v[u][q][i] = ok ? __ldcg(reinterpret_cast<const double2 *>(
+                                                          part + ((size_t)pr * kConsumerThreads + tid) * 16))
+                                                    : make_double2(0.0, 0.0);
+                                }
+                        }
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+#pragma unroll
+                            for (int q = 0; q < NC; ++q)
+#pragma unroll
+                                for (int i = 0; i < MB; ++i) {
+                                    acc[q][i][j][0] += v[u][q][i].x;
+                                    acc[q][i][j][1] += v[u][q][i].y;
+                                }
+                    }
+                }
+            } else {
+                for (int c = sk_g - 1; c >= c_lo; --c) {
+                    if (p.sk_begin[c + 1] <= p.sk_begin[c]) continue;      // (an empty CTA parks nothing)
                     const unsigned char *part = p.sk_part + (size_t)c * kPartBytes;
 #pragma unroll
                     for (int q = 0; q < NC; ++q)
@@ -487,7 +538,6 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                                 acc[q][i][j][1] += v.y;
                             }
                 }
-                if (cb <= tile_first) break;                           // CTA c held the tile's first slab
             }
         }
 
@@ -613,7 +663,12 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
     constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
     constexpr int Q = 8 * WARPS_N;                            // columns per quarter tile
     constexpr int QPT = C::BN / Q;                            // quarters per full tile (4)
-    constexpr int kMinWork = 4;                               // quarter slabs a stream-K CTA should at least get
+    // quarter slabs a stream-K CTA should at least get (CHASE_SK_MIN_WORK overrides; 0 disables stream-K: experiments)
+    static const int kMinWork = [] {
+        const char *env = std::getenv("CHASE_SK_MIN_WORK");
+        return env && env[0] ? std::atoi(env) : 4;
+    }();
+    if (kMinWork <= 0) allow_sk = false;
     const int KT = (int)((N + C::BK - 1) / C::BK);
     const int tiles_m = (int)((M + C::BM - 1) / C::BM);
     sms = std::max(1, std::min(sms, kMaxSkCtas));
@@ -715,6 +770,63 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
     pl.sk_begin[G] = (int)total_slabs;
 }
 
+// Stream-K scratch for launches that bring none (chase_hemm, chase_residuals, the row-sharded path): a small
+// per-process cache of device buffers.  A buffer is handed to one launch at a time: it becomes free again
+// when the event recorded behind that launch has completed, so launches on different streams never share
+// one, and nothing is allocated or freed in steady state.  (Not meant for stream capture: a captured event
+// record does not mark real completion.  chase_filter_ws uses the caller's workspace and is capturable.)
+struct SkSlot {
+    void *ptr;
+    cudaEvent_t ev;
+    int dev;
+    bool held;          // between acquire and release on some host thread
+    uint32_t epoch;
+};
+std::mutex g_sk_mu;
+std::vector<SkSlot> g_sk_slots;
+
+cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(g_sk_mu);
+    for (size_t i = 0; i < g_sk_slots.size(); ++i) {
+        SkSlot &sl = g_sk_slots[i];
+        if (sl.dev != dev || sl.held) continue;
+        const cudaError_t q = cudaEventQuery(sl.ev);
+        if (q == cudaErrorNotReady) continue;
+        if (q != cudaSuccess) return q;
+        sl.held = true;
+        *slot = (int)i; *ptr = sl.ptr; *epoch = ++sl.epoch;
+        return cudaSuccess;
+    }
+    SkSlot sl{};
+    sl.dev = dev; sl.held = true; sl.epoch = 1;
+    if ((e = cudaMalloc(&sl.ptr, dmma_sk_scratch_bytes())) != cudaSuccess) return e;
+    if ((e = cudaMemset(sl.ptr, 0, kSkFlagBytes)) != cudaSuccess ||
+        (e = cudaEventCreateWithFlags(&sl.ev, cudaEventDisableTiming)) != cudaSuccess) {
+        cudaFree(sl.ptr);
+        return e;
+    }
+    try {
+        g_sk_slots.push_back(sl);
+    } catch (const std::exception &) {
+        cudaEventDestroy(sl.ev);
+        cudaFree(sl.ptr);
+        return cudaErrorMemoryAllocation;
+    }
+    *slot = (int)g_sk_slots.size() - 1; *ptr = sl.ptr; *epoch = 1;
+    return cudaSuccess;
+}
+
+cudaError_t sk_cache_release(int slot, cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g_sk_mu);
+    SkSlot &sl = g_sk_slots[(size_t)slot];
+    const cudaError_t e = cudaEventRecord(sl.ev, stream);
+    sl.held = false;
+    return e;
+}
+
 template <bool CPLX>
 cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta, double c, int use_beta,
                    cudaStream_t stream, const double *c_col) {
@@ -740,16 +852,21 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     }
     const StepPlan &pl = plan->step_plan;
 
-    // Stream-K scratch: the caller's (chase_filter_ws: part of the workspace), else stream-ordered memory.
+    // Stream-K scratch: the caller's (chase_filter_ws: part of the workspace), else one of the library's
+    // cached buffers, handed out in stream order (sk_cache_*).
     unsigned char *scratch = (unsigned char *)plan->sk_scratch;
-    bool own_scratch = false;
+    int cache_slot = -1;
+    uint32_t epoch = 0;
     cudaError_t e;
-    if (pl.sk_ctas > 0 && !scratch) {
-        if ((e = cudaMallocAsync((void **)&scratch, dmma_sk_scratch_bytes(), stream)) != cudaSuccess) return e;
-        own_scratch = true;
-    }
-    if (pl.sk_ctas > 0 && (own_scratch || plan->sk_epoch == 0)) {       // flags start at 0, epochs at 1
-        if ((e = cudaMemsetAsync(scratch, 0, kSkFlagBytes, stream)) != cudaSuccess) return e;
+    if (pl.sk_ctas > 0) {
+        if (!scratch) {
+            if ((e = sk_cache_acquire(&cache_slot, (void **)&scratch, &epoch)) != cudaSuccess) return e;
+        } else {
+            if (plan->sk_epoch == 0 &&                                     // flags start at 0, epochs at 1
+                (e = cudaMemsetAsync(scratch, 0, kSkFlagBytes, stream)) != cudaSuccess)
+                return e;
+            epoch = ++plan->sk_epoch;
+        }
     }
 
     StepParams p;
@@ -770,7 +887,7 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     p.bn_w = pl.bn_w;
     p.dp_tiles = pl.dp_tiles;
     p.sk_ctas = pl.sk_ctas;
-    p.epoch = own_scratch ? 1u : ++plan->sk_epoch;
+    p.epoch = epoch;
     p.sk_flag = (uint32_t *)scratch;
     p.sk_part = scratch ? scratch + kSkFlagBytes : nullptr;
     p.alpha = alpha;
@@ -794,9 +911,11 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     cfg.numAttrs = 1;
     e = cudaLaunchKernelEx(&cfg, step_dmma_kernel<CPLX>, *mA, *mB, p);
     count_launch();
-    if (e != cudaSuccess) return e;
-    if (own_scratch) return cudaFreeAsync(scratch, stream);
-    return cudaSuccess;
+    if (cache_slot >= 0) {
+        const cudaError_t e2 = sk_cache_release(cache_slot, stream);
+        if (e == cudaSuccess) e = e2;
+    }
+    return e;
 }
 
 }  // namespace

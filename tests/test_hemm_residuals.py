@@ -82,10 +82,12 @@ def test_gpu_residuals_of_exact_eigenpairs():
 
 @pytest.mark.gpu
 @pytest.mark.parametrize("dtype", [torch.float32, torch.float64, torch.complex64, torch.complex128])
-@pytest.mark.parametrize("N,n", [(1040, 5), (203, 1), (777, 8), (1536, 3), (64, 7)])
+@pytest.mark.parametrize("N,n", [(1040, 5), (203, 1), (777, 8), (1536, 3), (64, 7), (2600, 2), (4100, 6), (130, 4)])
 def test_gpu_skinny_hemm_and_residuals(dtype, N, n):
-    """1..8 columns take the streaming kernel (csrc/step_skinny.cu): all dtypes, odd N, a chunk tail,
-    beta = 0 must not read Y, per-column shifts (residuals)."""
+    """1..8 columns take the streaming kernels (csrc/step_stream.cu: bulk-copy ring, when the columns of
+    H start on 16-byte boundaries; csrc/step_skinny.cu otherwise): all dtypes, odd N, several persistent
+    column blocks per CTA, ragged last block and last stage, beta = 0 must not read Y, per-column shifts
+    (residuals)."""
     tol = 1e-12 if dtype in (torch.complex128, torch.float64) else 2e-5
     H = W.hermitian_gaussian_ensemble(N, dtype, seed=91)
     X = W.gaussian_colmajor(N, n, dtype, seed=92)
