@@ -106,6 +106,9 @@ class ClockSampler:
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
+            t0 = time.perf_counter()          # short timed regions: make sure the sampler is already running
+            while not self.lines and time.perf_counter() - t0 < 3.0:
+                time.sleep(0.02)
         except OSError:
             self.proc = None
 
@@ -437,7 +440,7 @@ def cpu_blas_context(w, ncols: int = 128):
             "seconds": dt, "gflops": f * float(w.N) ** 2 * X.shape[1] / dt * 1e-9}
 
 
-ALL_CONFIG_STEPS = {1: 20, 2: 10, 3: 5, 5: 3}     # timed filter calls per non-headline config (3 warm-ups each)
+ALL_CONFIG_STEPS = {1: 1000, 2: 20, 3: 5, 5: 3}     # timed filter calls per non-headline config (3 warm-ups each)
 
 
 def run_other_configs(pkg, device, headline_cfg: int):

@@ -466,7 +466,19 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
             }
             continue;
         }
-        if (use_dmma) {
+        // Few active columns left (the tail of a sorted-degree schedule): one streaming pass over H beats a
+        // tensor tile that would be mostly padding (tcgen05 tiles are 128 / 256 columns wide; FP64: see
+        // launch_one_step for the measured crossover).
+        StepArgs ska;
+        ska.H = H;
+        ska.X = (const char *)buf[src] + (size_t)s * col_bytes;
+        ska.Y = (char *)buf[src ^ 1] + (size_t)s * col_bytes;
+        ska.N = N; ska.n = ncols - s;
+        ska.alpha = alpha[k]; ska.beta = beta[k]; ska.c = c; ska.use_beta = k > 1;
+        const bool few = ska.n <= (use_dmma ? 6 : kSkinnyMaxCols) && !(up && k == 1);
+        if ((use_dmma || use_tf32) && few && stream_supported(dtype, ska)) {
+            e = launch_step_stream(dtype, ska, stream);
+        } else if (use_dmma) {
             e = dmma_launch_step(&plan, src, s, alpha[k], beta[k], c, k > 1, stream);
         } else if (use_tf32) {
             e = tf32_launch_step(&tplan, src, s, alpha[k], beta[k], c, k > 1, stream);

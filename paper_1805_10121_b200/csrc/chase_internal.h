@@ -70,8 +70,8 @@ struct DmmaPlan {
     StepPlan step_plan;
 };
 bool dmma_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
-// Returns cudaSuccess, or an error (then the caller falls back to the generic kernels
-// only if the failure is "driver entry point unavailable"; anything else is reported).
+// Returns cudaSuccess or the error of the tensor-map encoding (reported to the caller; there is no
+// silent fallback to another kernel family).
 cudaError_t dmma_plan_create(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int64_t N,
                              void *V, void *W, int64_t ncols);
 // Row-sharded variant: H_loc is the nrows x N row block [row0, row0 + nrows) of H, column-major, ld = nrows.
@@ -93,6 +93,7 @@ struct Tf32Plan {
     int64_t N, ncols;
     void *buf[2];
     void *sync_ctr;                             // 4-byte counter of the producers' soft grid barrier
+    int pair;                                   // 1: CTA-pair kernel (cta_group::2, 256-row tiles), 0: single-CTA kernel
 };
 bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
 int tf32_vector_blocks(chase_dtype_t dtype);    // vector-sized blocks in the workspace besides H_lo

@@ -1,8 +1,9 @@
 // Generic FMA step kernel: any N, any number of active columns, all four dtypes.
 //   Y[:, j] <- alpha * (H X[:, j] - c X[:, j]) + beta * Y[:, j]       (Alg. 4 l.4 / l.9)
 // Shared-memory tiled GEMM on the FP32 / FP64 FMA pipes with the shift, scaling and V_{k-1}
-// term fused into the epilogue.  It is the path for float / complex<float>, and for sizes
-// the TMA + DMMA kernel does not take (N not a multiple of 8 complex / 16 real elements).
+// term fused into the epilogue.  It is the correctness path for the shapes neither tensor kernel takes
+// -- their TMA views need columns that start on 16-byte boundaries: float64 / complex64 with odd N,
+// float32 with N % 4 != 0 -- and for 9..31 active columns of a float32 / complex64 problem.
 #include "chase_internal.h"
 
 namespace chase {

@@ -33,6 +33,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <mutex>
 
 #include "chase_internal.h"
@@ -406,6 +407,266 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
     }
 }
 
+// ---------------------------------------------------------------- CTA-pair variant (cta_group::2)
+// Two CTAs of a cluster (the two SMs of a TPC) share one 256 x 256 tile: tcgen05.mma.cta_group::2 with
+// M = 256 takes 128 rows of A from each CTA's shared memory and HALF of B (128 of the 256 real columns)
+// from each, and leaves each CTA's 128 x 256 accumulator rows in its own TMEM.  Per CTA and stage the
+// tensor core then reads 48 KB of operands instead of 72 KB and the converter warps derive the lo (and,
+// complex, the rotated -iX) tiles of only 8 KB of B instead of 16 KB: the shared-memory port, which
+// bounded the single-CTA kernel at ~72 % tensor activity, drops below the MMA time.
+//   complex64: CTA 0 holds X (-> real parts), CTA 1 holds -iX (-> imaginary parts), both from the same
+//              raw X tile (CTA 1 rotates it in place); float32: each CTA holds its 128 columns of X.
+// Synchronisation: every CTA has its own TMA / empty / accumulator-full barriers (tcgen05.commit is
+// multicast to both); the barriers that gate the single MMA issuer (CTA 0) -- "converted" and
+// "accumulator drained" -- live in CTA 0 and take remote arrivals from CTA 1 (mapa + cluster-scope
+// release / acquire).
+constexpr int STAGES2 = 6;
+constexpr int BH = TN / 2;                       // real B columns held by one CTA of a pair
+constexpr int B2_BYTES = BH * KS * 4;            // 8 KB
+constexpr int STAGE2_BYTES = 2 * A_BYTES + 2 * B2_BYTES;   // A raw | A lo | B hi | B lo : 32 KB
+constexpr int SMEM2_TOTAL = STAGES2 * STAGE2_BYTES + 1024 + 512;
+constexpr uint32_t kInstrDesc2 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) |
+                                 ((uint32_t)((2 * TM) >> 4) << 24);
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+// Arrive on a barrier of the peer CTA.  Default (CTA-scope release) semantics, as for a local arrive: the
+// cluster-scope forms cost a MEMBAR.ALL.GPU per arrive and an L1 invalidation per wait (measured: 2000
+// instead of 830 clk per stage).  What the arrive publishes here is shared memory already fenced for the
+// async proxy (converters) or the completion of TMEM loads (accumulator warps), not global memory.
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) { mbar_wait(bar, parity); }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void umma_tf32_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDesc2), "r"(accumulate) : "memory");
+}
+// arrives (once the MMAs issued so far have retired) on the barrier at this offset in BOTH CTAs of the pair
+__device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+
+template <bool CPLX>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
+                      const Tf32Params p) {
+    constexpr int COLS = CPLX ? TN / 2 : TN;      // (complex or real) columns per pair tile
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bar_base = smem_base + STAGES2 * STAGE2_BYTES;   // full[S], empty[S], conv[S], tfull[2], tempty[2], tmem slot
+    const uint32_t bar_conv = bar_base + 8 * (2 * STAGES2);
+    const uint32_t bar_tfull = bar_base + 8 * (3 * STAGES2);
+    const uint32_t bar_tempty = bar_base + 8 * (3 * STAGES2 + 2);
+    const uint32_t tmem_slot = bar_base + 8 * (3 * STAGES2 + 4);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();              // 0: leader (issues the MMAs), 1: peer
+    const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
+    const int total_tiles = p.tiles_m * p.tiles_n;        // tiles of 256 rows
+    const int KT = (int)((p.KF + KS - 1) / KS);
+    const int NCH = (KT + CHUNK - 1) / CHUNK;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES2; ++s) {
+            mbar_init(bar_base + 8 * s, 1);                       // full: this CTA's producer (expect_tx)
+            mbar_init(bar_base + 8 * (STAGES2 + s), 1);           // empty: one multicast tcgen05.commit
+            mbar_init(bar_conv + 8 * s, 2 * kConvWarps);          // conv (used in CTA 0): converter warps of both CTAs
+        }
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(bar_tfull + 8 * b, 1);                      // chunk accumulator complete (multicast commit)
+            mbar_init(bar_tempty + 8 * b, 2 * kAccWarps);         // (used in CTA 0): drained by both CTAs' accumulator warps
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {   // all of TMEM in both CTAs: two 256-column fp32 accumulators (ping-pong between chunks)
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(2 * TN) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();                                     // barriers of both CTAs initialised before any remote arrive
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    uint32_t tmem_base;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ TMA producer (both CTAs)
+        if (lane == 0) {
+            const int syncs_per_tile = (KT + kSyncStages - 1) / kSyncStages;
+            unsigned it = 0;
+            unsigned *sync_ctr = p.sync_ctr;
+            int round = 0;
+            for (int tile = pair; tile < total_tiles; tile += npairs, ++round) {
+                int tile_m, tile_n;
+                tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+                const int m0 = tile_m * (2 * TM) + (int)rank * TM, n0 = tile_n * COLS;
+                const int nb0 = p.col0 + n0 + (CPLX ? 0 : (int)rank * BH);   // complex: both CTAs take the same raw X tile
+                const unsigned active = 2u * (unsigned)min(npairs, total_tiles - round * npairs);
+                const unsigned sync_base = (unsigned)round * gridDim.x * (unsigned)syncs_per_tile;
+                for (int kt = 0; kt < KT; ++kt, ++it) {
+                    if (sync_ctr && kt % kSyncStages == 0 &&
+                        !soft_grid_sync(sync_ctr, sync_base + active * (unsigned)(kt / kSyncStages + 1)))
+                        sync_ctr = nullptr;
+                    const int s = it % STAGES2;
+                    const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES2 + s);
+                    if (it >= STAGES2) mbar_wait(empty, ((it / STAGES2) - 1) & 1);
+                    const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sb_hi = sa_hi + 2 * A_BYTES;
+                    const int k0 = kt * KS;
+                    mbar_expect_tx(full, A_BYTES + B2_BYTES);
+                    tma_load_2d(sa_hi, &tmapA, full, k0, m0);
+                    tma_load_2d(sb_hi, &tmapB, full, k0, nb0);
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer (leader CTA only)
+        if (lane == 0 && rank == 0) {
+            unsigned it = 0, gc = 0;
+            for (int tile = pair; tile < total_tiles; tile += npairs) {
+                int kt = 0;
+                for (int ch = 0; ch < NCH; ++ch, ++gc) {
+                    const int b = gc & 1;
+                    if (gc >= 2) {   // the accumulator warps of BOTH CTAs must have drained this buffer's previous chunk
+                        mbar_wait_cluster(bar_tempty + 8 * b, ((gc >> 1) - 1) & 1);
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                    }
+                    const uint32_t d = tmem_base + b * TN;
+                    const int kt_end = min(KT, kt + CHUNK);
+                    for (bool first = true; kt < kt_end; ++kt, ++it) {
+                        const int s = it % STAGES2;
+                        mbar_wait(bar_base + 8 * s, (it / STAGES2) & 1);          // this CTA's TMA tiles landed
+                        mbar_wait_cluster(bar_conv + 8 * s, (it / STAGES2) & 1);  // lo / rot tiles written in both CTAs
+                                                                                  // (the peer's converters saw its TMA tiles)
+                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                        const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sa_lo = sa_hi + A_BYTES;
+                        const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B2_BYTES;
+#pragma unroll
+                        for (int ks = 0; ks < KS / 8; ++ks) {
+                            const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
+                            const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
+                            const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
+                            const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
+                            umma_tf32_pair(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
+                            umma_tf32_pair(d, al, bh, 1u);                 // lo * hi
+                            umma_tf32_pair(d, ah, bh, 1u);                 // hi * hi
+                            first = false;
+                        }
+                        umma_commit_pair(bar_base + 8 * (STAGES2 + s));   // frees the stage in both CTAs when these MMAs retire
+                    }
+                    umma_commit_pair(bar_tfull + 8 * b);                  // this chunk's accumulator is complete (both CTAs)
+                }
+            }
+        }
+    } else if (warp < 2 + kConvWarps) {
+        // ------------------------------------------------------------------ converter warps (both CTAs)
+        constexpr int CT = kConvWarps * 32;
+        constexpr int NA = A_BYTES / 16 / CT, NBV = B2_BYTES / 16 / CT;
+        const int ct = threadIdx.x - 64;
+        const uint32_t leader_conv = mapa_shared(bar_conv, 0);
+        unsigned it = 0;
+        for (int tile = pair; tile < total_tiles; tile += npairs) {
+            for (int kt = 0; kt < KT; ++kt, ++it) {
+                const int s = it % STAGES2;
+                mbar_wait(bar_base + 8 * s, (it / STAGES2) & 1);
+                const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sa_lo = sa_hi + A_BYTES;
+                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B2_BYTES;
+                float4 va[NA], vb[NBV];
+#pragma unroll
+                for (int i = 0; i < NA; ++i) va[i] = lds128(sa_hi + (uint32_t)(ct + i * CT) * 16);
+#pragma unroll
+                for (int i = 0; i < NBV; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
+#pragma unroll
+                for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
+                if (CPLX && rank == 1) {
+                    // this CTA supplies -iX: rotate the raw tile in place (a thread rewrites the chunk it read)
+#pragma unroll
+                    for (int i = 0; i < NBV; ++i) {
+                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
+                        sts128(sb_hi + off, rot_mi(vb[i]));
+                        sts128(sb_lo + off, rot_mi(split_lo(vb[i])));
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < NBV; ++i) sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, split_lo(vb[i]));
+                }
+                // generic-proxy writes -> visible to the tensor core's async-proxy reads
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(leader_conv + 8 * s);
+            }
+        }
+    } else if (warp >= kFirstAccWarp) {
+        // ------------------------------------------------------------------ accumulator / epilogue warps (both CTAs)
+        const int quarter = warp & 3;
+        const int half = (warp - kFirstAccWarp) >> 2;
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
+        const uint32_t leader_tempty = mapa_shared(bar_tempty, 0);
+        const float alpha = p.alpha, beta = p.beta;
+        unsigned gc = 0;
+        for (int tile = pair; tile < total_tiles; tile += npairs) {
+            int tile_m, tile_n;
+            tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+            const int m0 = tile_m * (2 * TM) + (int)rank * TM, n0 = tile_n * COLS;
+            float racc[TN / 2];
+#pragma unroll
+            for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
+            for (int ch = 0; ch < NCH; ++ch, ++gc) {
+                const int b = gc & 1;
+                mbar_wait(bar_tfull + 8 * b, (gc >> 1) & 1);
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+                for (int j = 0; j < TN / 2 / 32; ++j) {
+                    float t[32];
+                    tmem_ld32(taddr + b * TN + j * 32, t);
+#pragma unroll
+                    for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(leader_tempty + 8 * b);
+            }
+
+            const int64_t row = (int64_t)m0 + quarter * 32 + lane;
+            const bool row_ok = row < p.N;
+#pragma unroll
+            for (int i = 0; i < TN / 2; ++i) {
+                // complex: half 0 owns the real parts, half 1 the imaginary parts of columns n0 .. n0+127
+                const int col = CPLX ? n0 + i : n0 + half * (TN / 2) + i;
+                if (col < p.n && row_ok) {
+                    const float c = p.c_col ? (float)p.c_col[col] : p.c;
+                    const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
+                    float y = alpha * (racc[i] - c * p.X[off]);
+                    if (p.use_beta) y = fmaf(beta, p.Y[off], y);
+                    p.Y[off] = y;
+                }
+            }
+        }
+    }
+
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    cluster_sync_all();                                     // no CTA frees TMEM or exits while its peer may still signal it
+    if (warp == 1) {
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(2 * TN) : "memory");
+    }
+}
+
 // ---------------------------------------------------------------- host side
 using EncodeTiledFn = CUresult (*)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
@@ -455,6 +716,9 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] {
         attr_err = cudaFuncSetAttribute(step_tf32_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL);
+        if (attr_err == cudaSuccess)
+            attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            SMEM2_TOTAL);
     });
     if (attr_err != cudaSuccess) return attr_err;
     const int64_t n = plan->ncols - s;
@@ -470,7 +734,8 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     p.KF = plan->N * FL;
     p.n = (int)n;
     p.col0 = (int)s;
-    p.tiles_m = (int)((plan->N + TM - 1) / TM);
+    const bool pair = plan->pair != 0;
+    p.tiles_m = pair ? (int)((plan->N + 2 * TM - 1) / (2 * TM)) : (int)((plan->N + TM - 1) / TM);
     p.tiles_n = (int)((n + COLS - 1) / COLS);
     p.alpha = (float)alpha;
     p.beta = (float)beta;
@@ -479,11 +744,18 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     p.use_beta = use_beta;
     p.sync_ctr = (unsigned *)plan->sync_ctr;
     const int total_tiles = p.tiles_m * p.tiles_n;
-    const int grid = std::min(total_tiles, sm_count());      // persistent: one CTA per SM
     if (p.sync_ctr) {
         cudaError_t e = cudaMemsetAsync(p.sync_ctr, 0, sizeof(unsigned), stream);
         if (e != cudaSuccess) return e;
     }
+    if (pair) {   // persistent CTA pairs: one cluster of 2 per TPC
+        const int grid = 2 * std::min(total_tiles, std::max(1, sm_count() / 2));
+        step_tf32_pair_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM2_TOTAL, stream>>>(
+            *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
+        count_launch();
+        return cudaGetLastError();
+    }
+    const int grid = std::min(total_tiles, sm_count());      // persistent: one CTA per SM
     step_tf32_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM_TOTAL, stream>>>(
         *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
     count_launch();
@@ -512,11 +784,15 @@ cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H,
     plan->buf[0] = V;
     plan->buf[1] = workspace;
     plan->sync_ctr = (workspace && vb) ? (char *)workspace + vb : nullptr;
+    // CTA pairs (cta_group::2) unless CHASE_TF32_PAIR=0 asks for the single-CTA kernel (experiments / fallback)
+    const char *pair_env = std::getenv("CHASE_TF32_PAIR");
+    plan->pair = !(pair_env && pair_env[0] == '0');
     cudaError_t e;
     if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A, H, KF, N, TM)) != cudaSuccess) return e;
+    const int b_box = plan->pair ? TN / 2 : (cplx ? TN / 2 : TN);      // B columns one TMA box brings
     for (int i = 0; i < 2; ++i)
         if (plan->buf[i] &&
-            (e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], plan->buf[i], KF, ncols, cplx ? TN / 2 : TN)) != cudaSuccess)
+            (e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], plan->buf[i], KF, ncols, b_box)) != cudaSuccess)
             return e;
     return cudaSuccess;
 }
