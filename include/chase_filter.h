@@ -278,12 +278,16 @@ int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
 /* Work decomposition the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active`
  * columns of an N x N problem on a GPU with `sms` SMs (host only, no CUDA call; for tests and inspection).
- * out (HOST int32[6]) = {row tiles of 128, column tiles, column tile width, data-parallel tiles (one CTA
- * each, grouped raster order), stream-K CTAs, k-slabs per tile}.  The column tiles cover [0, n_active)
- * exactly once.  The tiles after the data-parallel ones are shared by the stream-K CTAs in contiguous
- * k-slab ranges: sk_begin (HOST int32[stream-K CTAs + 1], at most CHASE_MAX_SK_CTAS + 1; may be NULL)
- * receives the range boundaries, slab s being k-slab (s % slabs per tile) of tile (data-parallel tiles +
- * s / slabs per tile).  Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
+ * out (HOST int32[9]) = {row tiles of 128, column tiles, column tile width, data-parallel tiles, stream-K
+ * CTAs, k-slabs per tile, CTAs launched (`grid`), data-parallel rounds, first stream-K CTA}.  The column
+ * tiles cover [0, n_active) exactly once.  CTA b owns the whole tiles r * grid + b < data-parallel tiles
+ * (r < rounds) in grouped raster order: by default persistent CTAs (grid = sms, first stream-K CTA = 0,
+ * the producers kept in lock-step by a soft barrier); with CHASE_DMMA_LOCKSTEP=0 one tile per CTA (rounds = 1,
+ * the stream-K CTAs follow them: first stream-K CTA = data-parallel tiles).  The remaining tiles are shared
+ * by the CTAs first .. first + stream-K CTAs - 1 in contiguous k-slab ranges: sk_begin (HOST
+ * int32[stream-K CTAs + 1], at most CHASE_MAX_SK_CTAS + 1; may be NULL) receives the range boundaries, slab s
+ * being k-slab (s % slabs per tile) of tile (data-parallel tiles + s / slabs per tile).
+ * Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
 #define CHASE_MAX_SK_CTAS 160
 int chase_filter_step_plan(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out,
                            int32_t *sk_begin);

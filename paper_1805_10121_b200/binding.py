@@ -250,12 +250,13 @@ def chase_filter_schedule(degrees: Sequence[int]):
 
 def chase_filter_step_plan(N: int, n_active: int, dtype: torch.dtype, sms: int = 148):
     """Work decomposition of one FP64 tensor-kernel launch: dict with tiles_m, tiles_n, tile_width,
-    dp_tiles, sk_ctas, slabs_per_tile and sk_begin (numpy int32[sk_ctas + 1])."""
-    out = np.zeros(6, dtype=np.int32)
+    dp_tiles, sk_ctas, slabs_per_tile, grid, dp_rounds and sk_begin (numpy int32[sk_ctas + 1])."""
+    out = np.zeros(9, dtype=np.int32)
     skb = np.zeros(161, dtype=np.int32)
     _check(load().chase_filter_step_plan(int(N), int(n_active), _DTYPE_CODE[dtype], int(sms), out.ctypes.data,
                                          skb.ctypes.data))
-    keys = ("tiles_m", "tiles_n", "tile_width", "dp_tiles", "sk_ctas", "slabs_per_tile")
+    keys = ("tiles_m", "tiles_n", "tile_width", "dp_tiles", "sk_ctas", "slabs_per_tile", "grid", "dp_rounds",
+            "sk_first")
     plan = {k: int(v) for k, v in zip(keys, out)}
     plan["sk_begin"] = skb[: plan["sk_ctas"] + 1].copy()
     return plan

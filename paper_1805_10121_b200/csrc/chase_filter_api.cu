@@ -348,6 +348,7 @@ int chase_filter_step_plan(int64_t N, int64_t n_active, chase_dtype_t dtype, int
         return (int)cudaErrorMemoryAllocation;
     }
     out[0] = pl.tiles_m; out[1] = pl.tiles_n; out[2] = pl.bn_w; out[3] = pl.dp_tiles; out[4] = pl.sk_ctas; out[5] = pl.KT;
+    out[6] = pl.grid; out[7] = pl.dp_rounds; out[8] = pl.sk_first;
     if (sk_begin)
         for (int g = 0; g <= pl.sk_ctas; ++g) sk_begin[g] = pl.sk_begin[g];
     return CHASE_OK;

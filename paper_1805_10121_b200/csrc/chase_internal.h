@@ -37,13 +37,18 @@ cudaError_t launch_step_stream(chase_dtype_t dtype, const StepArgs &a, cudaStrea
 
 // TMA + DMMA tensor kernels (CHASE_C128 with any N >= 16, CHASE_F64 with even N).
 // Work decomposition of one launch on `n` active columns (csrc/step_dmma.cu): tiles of
-// 128 rows x bn_w columns in grouped raster order; the first dp_tiles tiles get one CTA each, the k-slabs
-// of the remaining tiles are shared by sk_ctas stream-K CTAs: CTA g owns slabs [sk_begin[g], sk_begin[g+1])
-// of that region, slab s = k-slab (s % KT) of tile dp_tiles + s / KT.
+// 128 rows x bn_w columns in grouped raster order; `grid` persistent CTAs; CTA b owns the whole tiles
+// r * grid + b (r < dp_rounds) of the first dp_tiles tiles, then CTAs 0 .. sk_ctas-1 share the k-slabs of the
+// remaining tiles: CTA g owns slabs [sk_begin[g], sk_begin[g+1]) of that region, slab s = k-slab (s % KT) of
+// tile dp_tiles + s / KT.
 constexpr int kMaxSkCtas = 160;                 // >= SM count of any sm_100 part
-constexpr size_t kSkFlagBytes = 1024;           // kMaxSkCtas uint32 flags, padded
+constexpr size_t kSkFlagBytes = 1024;           // kMaxSkCtas uint32 flags + the soft-barrier counter, padded
+constexpr size_t kSkSyncOffset = 800;           // byte offset of the soft-barrier counter inside the flag block
 struct StepPlan {
     int KT, tiles_m, tiles_n, bn_w, dp_tiles, sk_ctas;
+    int grid, dp_rounds;                        // CTAs launched; whole-tile rounds per CTA (tile r * grid + b)
+    int ragged_last;                            // raster variant: the last tile column after all others (lock-step mode)
+    int sk_first;                               // blockIdx of stream-K CTA 0 (0: persistent CTAs; dp_tiles: one CTA per whole tile)
     int sk_begin[kMaxSkCtas + 1];
 };
 // Bytes of device scratch the stream-K CTAs need (flags + one partial accumulator tile per CTA).
@@ -66,6 +71,7 @@ struct DmmaPlan {
     void *sk_scratch;                           // dmma_sk_scratch_bytes() of device memory, or null: every launch that
                                                 // needs it then takes stream-ordered memory (cudaMallocAsync)
     uint32_t sk_epoch;                          // flag value of the last stream-K launch on sk_scratch (0: flags not yet zeroed)
+    unsigned sync_count;                        // arrivals the soft-barrier counter in sk_scratch has seen so far
     int64_t step_plan_n;                        // active width step_plan was made for (-1: none)
     StepPlan step_plan;
 };

@@ -19,8 +19,12 @@
 // fragment load is bank-conflict free under the swizzle (complex: k = 8q + 2t + a; real:
 // k = {0,10,4,14}[t] ^ a with 16-byte loads shared by two MMAs), identically for A and B.
 //
-// Work decomposition of one launch (DESIGN.md 6.1 "stream-K tail"): the first `dp_tiles` CTAs own one
-// whole output tile each (data-parallel, grouped raster); the last `sk_ctas` CTAs share the remaining
+// Work decomposition of one launch (DESIGN.md 6.1 "stream-K tail").  Default (lock-step): persistent CTAs, one
+// per SM; CTA b owns the whole output tiles b, b + grid, ... of the first `dp_tiles` tiles (grouped raster), and
+// the producers of all CTAs keep within a window of 64 k-slabs of each other through a soft barrier, so that
+// they hit each other's H / X tiles in L2 (cfg 4: 153 instead of 325 GB of DRAM reads per step, 27 W less, same
+// speed).  CHASE_DMMA_LOCKSTEP=0: one CTA per whole tile, dispatched to whichever SM frees first.
+// In both modes `sk_ctas` CTAs then share the remaining
 // tiles' k-slabs in equal-TIME contiguous ranges (stream-K): a CTA whose range ends inside a tile
 // leaves its partial accumulators in the scratch buffer and raises a flag -- first thing, because it
 // walks its range from the top down --, the CTA that holds the tile's last slab adds the partials of
@@ -136,9 +140,15 @@ struct StepParams {
     int n;               // active columns
     int col0;            // first active column in the full buffer (TMA coordinate offset)
     int tiles_m, tiles_n;
+    int ragged_last;     // raster variant (tile_coords)
     int bn_w;            // column tile width of this launch: a multiple of 8 * WARPS_N, <= BN
-    int dp_tiles;        // tiles [0, dp_tiles) in raster order: one CTA each
-    int sk_ctas;         // stream-K CTAs covering tiles [dp_tiles, tiles_m * tiles_n)
+    int dp_tiles;        // tiles [0, dp_tiles) in raster order: whole tiles, tile r * gridDim.x + b belongs to CTA b
+    int dp_rounds;       // data-parallel rounds per CTA
+    int sk_first;        // first stream-K CTA: 0 (persistent CTAs: whole tiles first, then a stream-K range) or
+                         // dp_tiles (one CTA per whole tile, dispatched first; the stream-K CTAs follow)
+    int sk_ctas;         // CTAs [sk_first, sk_first + sk_ctas) share the k-slabs of tiles [dp_tiles, tiles_m * tiles_n)
+    unsigned *sync_ctr;  // soft barrier of the producers during the data-parallel rounds (or null)
+    unsigned sync_base;  // value of *sync_ctr before this launch
     uint32_t epoch;      // value the stream-K flags take in this launch
     unsigned char *sk_part;   // sk_ctas partial tiles of kPartBytes
     uint32_t *sk_flag;        // sk_ctas flags
@@ -149,16 +159,29 @@ struct StepParams {
                                     // slab s = k-slab (s % KT) of tile dp_tiles + s / KT
 };
 
-// Grouped rasterisation: consecutive CTAs cover kGroupN column tiles x a run of row tiles, so the
-// CTAs resident at one time share both H row panels and X column panels in L2.  kGroupN is chosen
-// so that a wave of 148 CTAs is roughly square in BYTES (rows*BM ~ cols*BN), which minimises the
+// Grouped rasterisation: consecutive tiles cover kGroupN column tiles x a run of row tiles, so the
+// CTAs working at one time share both H row panels and X column panels in L2.  kGroupN is chosen
+// so that a round of 148 tiles is roughly square in BYTES (rows*BM ~ cols*BN), which minimises the
 // DRAM traffic of 148 register-resident output tiles.
+// ragged_last (lock-step mode): the last tile column -- the only one that can be ragged, i.e. cheaper --
+// comes after all the others, so that the whole-tile rounds consist of equal-cost tiles that can walk along
+// k in step (with static ownership, interleaved cheap tiles would leave their owners idle at the barrier).
+// Without lock-step the ragged tiles stay interleaved: their H panels are then shared with the neighbours in
+// L2 and their bandwidth appetite (same H bytes for a quarter of the MMAs) is diluted among full tiles.
 template <int kGroupN>
-__host__ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int &tm, int &tn) {
+__host__ __device__ __forceinline__ void tile_coords(int t, int tiles_m, int tiles_n, int ragged_last, int &tm,
+                                                     int &tn) {
+    const int body_n = ragged_last ? tiles_n - 1 : tiles_n;
+    const int body = body_n * tiles_m;
+    if (t >= body) {
+        tm = t - body;
+        tn = body_n;
+        return;
+    }
     const int per_group = kGroupN * tiles_m;
     const int grp = t / per_group;
     const int first_n = grp * kGroupN;
-    const int gn = (tiles_n - first_n) < kGroupN ? (tiles_n - first_n) : kGroupN;
+    const int gn = (body_n - first_n) < kGroupN ? (body_n - first_n) : kGroupN;
     const int r = t - grp * per_group;
     tm = r / gn;
     tn = first_n + r % gn;
@@ -277,27 +300,57 @@ __device__ __forceinline__ void mainloop(double (&acc)[CPLX ? 2 : 1][Cfg<CPLX>::
 struct Segment {
     int tile, k0, k1;
 };
-// Next segment of this CTA (DP CTAs have exactly one); false when the CTA's work is exhausted.
-// A stream-K CTA walks its slab range [s_begin, s_end) from the TOP DOWN: the head of the last tile it
-// touches comes first -- it is parked at once for the higher-numbered CTA that holds that tile's tail --
+// Iterator over the segments of this CTA: first its whole tiles (one per data-parallel round), then its
+// stream-K range.  The stream-K range [s_begin, s_end) is walked from the TOP DOWN: the head of the last tile
+// it touches comes first -- it is parked at once for the higher-numbered CTA that holds that tile's tail --
 // and the tail of the first tile comes last, when the partial sums of the lower-numbered CTAs that hold
 // its head have long been parked.  (Bottom-up, every CTA would wait for the END of its predecessor.)
-__device__ __forceinline__ bool next_segment(const StepParams &p, int KT, bool is_dp, int s_begin, int &s_end,
-                                             Segment &seg) {
-    if (is_dp) {
-        if (s_end != 0) return false;
-        seg.tile = blockIdx.x; seg.k0 = 0; seg.k1 = KT;
-        s_end = 1;
-        return true;
+struct WorkIter {
+    int round, s_begin, s_end;
+};
+__device__ __forceinline__ WorkIter work_begin(const StepParams &p) {
+    WorkIter w;
+    w.round = 0;
+    w.s_begin = w.s_end = 0;
+    const int g = (int)blockIdx.x - p.sk_first;
+    if (g >= 0 && g < p.sk_ctas) { w.s_begin = p.sk_begin[g]; w.s_end = p.sk_begin[g + 1]; }
+    return w;
+}
+// false when the CTA's work is exhausted; `dp_round` = the round of a whole-tile segment, -1 for stream-K
+__device__ __forceinline__ bool next_segment(const StepParams &p, int KT, WorkIter &w, Segment &seg, int &dp_round) {
+    while (w.round < p.dp_rounds) {
+        const int t = w.round * (int)gridDim.x + (int)blockIdx.x;
+        dp_round = w.round++;
+        if (t < p.dp_tiles) {
+            seg.tile = t; seg.k0 = 0; seg.k1 = KT;
+            return true;
+        }
     }
-    if (s_end <= s_begin) return false;
-    const int tr = (s_end - 1) / KT;
+    dp_round = -1;
+    if (w.s_end <= w.s_begin) return false;
+    const int tr = (w.s_end - 1) / KT;
     const int tile_first = tr * KT;
     seg.tile = p.dp_tiles + tr;
-    seg.k1 = s_end - tile_first;
-    seg.k0 = max(s_begin, tile_first) - tile_first;
-    s_end = tile_first + seg.k0;
+    seg.k1 = w.s_end - tile_first;
+    seg.k0 = max(w.s_begin, tile_first) - tile_first;
+    w.s_end = tile_first + seg.k0;
     return true;
+}
+
+// Soft barrier between the TMA producers of all CTAs (a performance hint, never needed for correctness):
+// arrive on a global counter, then poll until `target` arrivals for a bounded time.  Returns false when
+// the wait timed out; the caller then stops polling but keeps arriving, so the counts stay consistent.
+constexpr int kSyncSlabs = 32;
+__device__ __forceinline__ bool soft_grid_sync(unsigned *ctr, unsigned target, bool poll) {
+    atomicAdd(ctr, 1u);
+    if (!poll) return false;
+    for (int i = 0; i < 4096; ++i) {
+        unsigned v;
+        asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+        if ((int)(v - target) >= 0) return true;
+        __nanosleep(32);
+    }
+    return false;
 }
 
 template <bool CPLX>
@@ -317,10 +370,8 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int KT = (int)((p.N + BK - 1) / BK);
-    const bool is_dp = (int)blockIdx.x < p.dp_tiles;
-    const int sk_g = (int)blockIdx.x - p.dp_tiles;
-    int s_begin = 0, s_end = 0;
-    if (!is_dp) { s_begin = p.sk_begin[sk_g]; s_end = p.sk_begin[sk_g + 1]; }
+    const int sk_g = (int)blockIdx.x - p.sk_first;    // index among the stream-K CTAs
+    WorkIter work = work_begin(p);
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) {
@@ -341,13 +392,25 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
         if (warp == kConsumerWarps && lane == 0) {
             // H is never written, so its first tiles may be fetched before the previous launch (which
             // produces this step's X) has finished; X loads and everything after wait for it.
-            bool dep_waited = false;
+            bool dep_waited = false, sync_poll = true;
+            const int spt = (KT + kSyncSlabs - 1) / kSyncSlabs;      // soft-barrier points per whole tile
             uint32_t it = 0;
             Segment seg;
-            while (next_segment(p, KT, is_dp, s_begin, s_end, seg)) {
+            int dp_round;
+            while (next_segment(p, KT, work, seg, dp_round)) {
                 int tile_m, tile_n;
-                tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+                tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, p.ragged_last, tile_m, tile_n);
                 const int m0 = tile_m * BM, n0 = tile_n * p.bn_w;
+                // data-parallel rounds: every kSyncSlabs slabs a producer checks in and waits (bounded) until ALL
+                // producers have passed the PREVIOUS check-in: nobody runs more than 2 * kSyncSlabs slabs ahead
+                // of the slowest CTA -- the union stream of that window (~35 MB) stays in L2 -- and nobody stalls
+                // unless it is a full window ahead.  (Meeting at every check-in cost 0.7 % of cfg 4.)
+                auto sync_point = [&](int kt) {
+                    if (dp_round >= 0 && p.sync_ctr && kt % kSyncSlabs == 0) {
+                        const unsigned q = (unsigned)(dp_round * spt + kt / kSyncSlabs);
+                        sync_poll = soft_grid_sync(p.sync_ctr, p.sync_base + gridDim.x * q, sync_poll);
+                    }
+                };
                 auto load_A = [&](uint32_t slot, int kt) {
                     const uint32_t full = bar_base + 8 * slot;
                     const uint32_t sa = smem_base + slot * S::STAGE_BYTES;
@@ -381,7 +444,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                 int kt = seg.k0;
                 if (!dep_waited) {
                     const int pre = min(STAGES, seg.k1 - seg.k0);       // ring is empty: no empty-wait needed
-                    for (int i = 0; i < pre; ++i) load_A(i, kt + i);
+                    for (int i = 0; i < pre; ++i) { sync_point(kt + i); load_A(i, kt + i); }
                     asm volatile("griddepcontrol.wait;" ::: "memory");
                     for (int i = 0; i < pre; ++i) load_B(i, kt + i);
                     dep_waited = true;
@@ -389,6 +452,7 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                     it += pre;
                 }
                 for (; kt < seg.k1; ++kt, ++it) {
+                    sync_point(kt);
                     const uint32_t slot = it % STAGES;
                     if (it >= (uint32_t)STAGES) mbar_wait(bar_base + 8 * (STAGES + slot), ((it / STAGES) - 1) & 1);
                     load_A(slot, kt);
@@ -412,12 +476,13 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 
     uint32_t it = 0;
     Segment seg;
-    while (next_segment(p, KT, is_dp, s_begin, s_end, seg)) {
+    int dp_round;
+    while (next_segment(p, KT, work, seg, dp_round)) {
         // Column tiling: tiles of bn_w columns; a tile with `ncols_tile` valid columns only
         // computes its first ceil(ncols_tile / 8) 8-column MMA blocks; block nb belongs to warp column
         // nb % WARPS_N, so the work stays balanced over the warps and the tile's time is ~ ceil(nblk / WARPS_N).
         int tile_m, tile_n;
-        tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
+        tile_coords<C::GROUP_N>(seg.tile, p.tiles_m, p.tiles_n, p.ragged_last, tile_m, tile_n);
         const int m0 = tile_m * BM, n0 = tile_n * p.bn_w;
         const int ncols_tile = min(p.bn_w, p.n - n0);
         const int nblk = (ncols_tile + 7) >> 3;
@@ -691,24 +756,43 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
         return (nblk + WARPS_N - 1) / WARPS_N;
     };
     const int q_full = quarters_of_col_tile(0), q_last = quarters_of_col_tile(tiles_n - 1);
+    static const bool lockstep_env = [] {          // default on; CHASE_DMMA_LOCKSTEP=0 selects one CTA per whole tile
+        const char *env = std::getenv("CHASE_DMMA_LOCKSTEP");
+        return !(env && env[0] == '0');
+    }();
+    // lock-step only pays (and only applies) when there are whole-tile rounds: same condition as D > 0 below
+    const bool lockstep = lockstep_env && allow_sk && T >= 2 * (int64_t)sms;
     auto quarters_of_tile = [&](int64_t t) {
         int tm, tn;
-        tile_coords<C::GROUP_N>((int)t, tiles_m, tiles_n, tm, tn);
+        tile_coords<C::GROUP_N>((int)t, tiles_m, tiles_n, lockstep ? 1 : 0, tm, tn);
         return tn == tiles_n - 1 ? q_last : q_full;
     };
-    pl.KT = KT; pl.tiles_m = tiles_m; pl.tiles_n = tiles_n; pl.bn_w = w;
+    pl.KT = KT; pl.tiles_m = tiles_m; pl.tiles_n = tiles_n; pl.bn_w = w; pl.ragged_last = lockstep ? 1 : 0;
     pl.dp_tiles = (int)T; pl.sk_ctas = 0; pl.sk_begin[0] = 0;
+    pl.grid = (int)T; pl.dp_rounds = 1; pl.sk_first = 0;      // default: one CTA per tile
     (void)QPT;
     if (!allow_sk || T <= 0) return;
 
-    // Data-parallel region: whole waves, all but the last one-to-two waves' worth of tiles.
+    // Data-parallel region: whole rounds of `sms` tiles, all but the last one-to-two rounds' worth of tiles.
     int64_t D = 0;
     if (T >= 2 * (int64_t)sms) D = (T / sms - 1) * sms;
-    // SM free times after the data-parallel region (list scheduling in blockIdx order), ascending: the g-th
-    // stream-K CTA is the (D + g)-th CTA of the grid and starts on the g-th SM to become free.
+    // Stream-K region: tiles [D, T); work in quarter slabs.  It must hold at least one round's worth of full
+    // tiles, or the CTAs could not all be made to finish together (the cheap ragged tiles come last).
+    double work = 0.0;
+    for (int64_t t = D; t < T; ++t) work += (double)quarters_of_tile(t) * KT;
+    while (D > 0 && work < (double)sms * q_full * KT) {
+        for (int64_t t = D - sms; t < D; ++t) work += (double)quarters_of_tile(t) * KT;
+        D -= sms;
+    }
+    // Time (quarter slabs) at which the SM that runs stream-K CTA g has finished its whole tiles.
+    //   lock-step: CTA b owns the tiles b, b + sms, ... and continues with stream-K range b;
+    //   default:   tiles go to whichever SM frees first (list scheduling in blockIdx order), and the g-th
+    //              stream-K CTA, the (D + g)-th CTA of the grid, starts on the g-th SM to become free.
     std::vector<double> free_at((size_t)sms, 0.0);
-    if (D > 0) {
-        if (q_last == q_full) {
+    if (lockstep) {
+        for (int64_t t = 0; t < D; ++t) free_at[(size_t)(t % sms)] += (double)quarters_of_tile(t) * KT;
+    } else if (D > 0) {
+        if (q_last == q_full) {                                               // all whole tiles cost the same
             std::fill(free_at.begin(), free_at.end(), (double)(D / sms) * q_full * KT);
         } else {
             std::priority_queue<double, std::vector<double>, std::greater<double>> heap;
@@ -721,9 +805,6 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
             for (int i = 0; i < sms; ++i) { free_at[(size_t)i] = heap.top(); heap.pop(); }
         }
     }
-    // Stream-K region: tiles [D, T); work in quarter slabs.
-    double work = 0.0;
-    for (int64_t t = D; t < T; ++t) work += (double)quarters_of_tile(t) * KT;
     int G = sms;
     if (work < (double)G * kMinWork) G = (int)std::max(1.0, work / kMinWork);
     const int64_t R = T - D;
@@ -731,23 +812,32 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
         // tiny launch: align the split with the tile boundaries (every CTA inside ONE tile)
         G = (int)(R * (G / R));
     }
-    if (G <= 1) return;                                        // too little work to split: one CTA per tile
+    if (D == 0 && G <= 1) return;                              // too little work to split: one CTA per tile
     if (D == 0 && R == G && q_last == q_full) return;          // one whole tile per CTA already: nothing to balance
-    // Water-filling: finish time F with sum_g max(0, F - free_at[g]) = work.
+    if (D > 0) G = sms;
+    // Water-filling: finish time F with sum_b max(0, F - free_at[b]) = work over the CTAs 0 .. G-1.
     double F = 0.0;
     {
+        std::vector<double> f(free_at.begin(), free_at.begin() + G);
+        std::sort(f.begin(), f.end());
         double acc_f = 0.0;
-        int used = 0;
-        for (int gI = 0; gI < G; ++gI) {          // free_at ascending: try using CTAs 0..gI
-            acc_f += free_at[(size_t)gI];
-            used = gI + 1;
-            F = (work + acc_f) / used;
-            if (gI + 1 == G || F <= free_at[(size_t)gI + 1]) break;
+        for (int i = 0; i < G; ++i) {                         // ascending: try using the i + 1 earliest CTAs
+            acc_f += f[(size_t)i];
+            F = (work + acc_f) / (i + 1);
+            if (i + 1 == G || F <= f[(size_t)i + 1]) break;
         }
-        (void)used;
     }
     pl.dp_tiles = (int)D;
     pl.sk_ctas = G;
+    if (lockstep || D == 0) {
+        pl.grid = D > 0 ? sms : G;
+        pl.dp_rounds = (int)(D / sms);
+        pl.sk_first = 0;
+    } else {
+        pl.grid = (int)D + G;
+        pl.dp_rounds = 1;
+        pl.sk_first = (int)D;
+    }
     // Boundaries: walk the region's tiles, cutting where the cumulative cost reaches each CTA's share.
     const int64_t total_slabs = R * KT;
     double target = 0.0, cum = 0.0;            // cost before the current tile
@@ -781,11 +871,12 @@ struct SkSlot {
     int dev;
     bool held;          // between acquire and release on some host thread
     uint32_t epoch;
+    unsigned sync_count;   // arrivals the soft-barrier counter in this buffer has seen so far
 };
 std::mutex g_sk_mu;
 std::vector<SkSlot> g_sk_slots;
 
-cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch) {
+cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch, unsigned *sync_base, unsigned sync_arrivals) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -798,10 +889,13 @@ cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch) {
         if (q != cudaSuccess) return q;
         sl.held = true;
         *slot = (int)i; *ptr = sl.ptr; *epoch = ++sl.epoch;
+        *sync_base = sl.sync_count;
+        sl.sync_count += sync_arrivals;
         return cudaSuccess;
     }
     SkSlot sl{};
-    sl.dev = dev; sl.held = true; sl.epoch = 1;
+    sl.dev = dev; sl.held = true; sl.epoch = 1; sl.sync_count = sync_arrivals;
+    *sync_base = 0;
     if ((e = cudaMalloc(&sl.ptr, dmma_sk_scratch_bytes())) != cudaSuccess) return e;
     if ((e = cudaMemset(sl.ptr, 0, kSkFlagBytes)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&sl.ev, cudaEventDisableTiming)) != cudaSuccess) {
@@ -852,20 +946,28 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     }
     const StepPlan &pl = plan->step_plan;
 
-    // Stream-K scratch: the caller's (chase_filter_ws: part of the workspace), else one of the library's
-    // cached buffers, handed out in stream order (sk_cache_*).
+    // Scratch (stream-K flags and partial tiles, soft-barrier counter): the caller's (chase_filter_ws: part of
+    // the workspace), else one of the library's cached buffers, handed out in stream order (sk_cache_*).
     unsigned char *scratch = (unsigned char *)plan->sk_scratch;
     int cache_slot = -1;
     uint32_t epoch = 0;
+    unsigned sync_base = 0;
+    const bool want_sync = pl.dp_rounds >= 1 && pl.sk_ctas > 0 && pl.sk_first == 0;   // persistent CTAs with whole-tile rounds
+    const unsigned sync_arrivals =
+        want_sync ? (unsigned)pl.grid * (unsigned)pl.dp_rounds * (unsigned)((pl.KT + kSyncSlabs - 1) / kSyncSlabs) : 0u;
     cudaError_t e;
     if (pl.sk_ctas > 0) {
         if (!scratch) {
-            if ((e = sk_cache_acquire(&cache_slot, (void **)&scratch, &epoch)) != cudaSuccess) return e;
-        } else {
-            if (plan->sk_epoch == 0 &&                                     // flags start at 0, epochs at 1
-                (e = cudaMemsetAsync(scratch, 0, kSkFlagBytes, stream)) != cudaSuccess)
+            if ((e = sk_cache_acquire(&cache_slot, (void **)&scratch, &epoch, &sync_base, sync_arrivals)) != cudaSuccess)
                 return e;
+        } else {
+            if (plan->sk_epoch == 0) {                                     // flags and counter start at 0, epochs at 1
+                if ((e = cudaMemsetAsync(scratch, 0, kSkFlagBytes, stream)) != cudaSuccess) return e;
+                plan->sync_count = 0;
+            }
             epoch = ++plan->sk_epoch;
+            sync_base = plan->sync_count;
+            plan->sync_count += sync_arrivals;
         }
     }
 
@@ -884,9 +986,14 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     p.col0 = (int)s;
     p.tiles_m = pl.tiles_m;
     p.tiles_n = pl.tiles_n;
+    p.ragged_last = pl.ragged_last;
     p.bn_w = pl.bn_w;
     p.dp_tiles = pl.dp_tiles;
+    p.dp_rounds = pl.dp_rounds;
+    p.sk_first = pl.sk_first;
     p.sk_ctas = pl.sk_ctas;
+    p.sync_ctr = want_sync && scratch ? (unsigned *)(scratch + kSkSyncOffset) : nullptr;
+    p.sync_base = sync_base;
     p.epoch = epoch;
     p.sk_flag = (uint32_t *)scratch;
     p.sk_part = scratch ? scratch + kSkFlagBytes : nullptr;
@@ -900,7 +1007,7 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     const CUtensorMap *mB = (const CUtensorMap *)plan->tmap_B[src];
 
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)(pl.dp_tiles + pl.sk_ctas));
+    cfg.gridDim = dim3((unsigned)pl.grid);
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = Smem<CPLX>::TOTAL;
     cfg.stream = stream;
@@ -948,6 +1055,7 @@ static void plan_common(DmmaPlan *plan, chase_dtype_t dtype, const void *H, int6
     plan->buf[1] = W;
     plan->sk_scratch = nullptr;
     plan->sk_epoch = 0;
+    plan->sync_count = 0;
     plan->step_plan_n = -1;
 }
 

@@ -215,3 +215,65 @@ def test_peak_probes_run():
     dmma = pkg.chase_fp64_peak_probe(1, 2048)
     print(f"FP64 peak probes: DFMA {dfma:.0f} GFLOP/s, DMMA {dmma:.0f} GFLOP/s")
     assert dfma > 1000 and dmma > 1000
+
+
+_LOCKSTEP_SCRIPT = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, {root!r}); sys.path.insert(0, {tests!r})
+import oracle, paper_1805_10121_b200 as pkg
+from paper_1805_10121_b200 import workloads as W
+N, n = 2048, 1317
+plan = pkg.chase_filter_step_plan(N, n, torch.complex128, torch.cuda.get_device_properties(0).multi_processor_count)
+assert plan["sk_first"] == plan["dp_tiles"] > 0 and plan["dp_rounds"] == 1, plan   # one CTA per whole tile, then stream-K
+w = W.make_config(4, N=N, ncols=n)
+w.degrees = torch.clamp(w.degrees // 6, min=1).to(torch.int32)            # sorted degrees 1..6: several column drops
+dev = torch.device("cuda:0")
+H = W.empty_colmajor(N, N, w.dtype, dev); H.copy_(w.H)
+V = W.empty_colmajor(N, n, w.dtype, dev); V.copy_(w.V0)
+ws = torch.empty(pkg.chase_filter_workspace_bytes(N, n, w.dtype), dtype=torch.uint8, device=dev); ws.fill_(0xFF)
+pkg.chase_filter_ws(H, V, w.degrees, w.a, w.b, w.lambda1, ws)
+torch.cuda.synchronize()
+ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), w.degrees.numpy(), w.a, w.b, w.lambda1)
+err = float(np.linalg.norm(V.cpu().numpy() - ref) / np.linalg.norm(ref))
+print("LOCKSTEP_ERR", err)
+assert err <= 1e-12
+"""
+
+
+def test_dynamic_mode_one_cta_per_whole_tile():
+    """CHASE_DMMA_LOCKSTEP=0 (one CTA per whole tile dispatched dynamically, stream-K CTAs behind them; the
+    default is persistent CTAs in lock-step, which every other test exercises) gives the same result as
+    the oracle.  The switch is read once per process, hence the subprocess."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, CHASE_DMMA_LOCKSTEP="0")
+    r = subprocess.run([sys.executable, "-c", _LOCKSTEP_SCRIPT.format(root=root, tests=os.path.join(root, "tests"))],
+                       env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    assert "LOCKSTEP_ERR" in r.stdout
+
+
+def test_default_mode_whole_tile_rounds_then_stream_k():
+    """Default plan on a shape with whole-tile rounds (336 tiles for 148 SMs): persistent CTAs, soft barrier
+    between the producers, ragged tile column last, then the stream-K ranges -- against the oracle, with
+    several column drops and NaN-filled scratch."""
+    import oracle
+    N, n = 2048, 1317
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    plan = pkg.chase_filter_step_plan(N, n, torch.complex128, sms)
+    assert plan["sk_first"] == 0 and plan["dp_rounds"] >= 1 and plan["grid"] == sms, plan
+    w = W.make_config(4, N=N, ncols=n)
+    w.degrees = torch.clamp(w.degrees // 6, min=1).to(torch.int32)
+    dev = torch.device("cuda:0")
+    H = W.empty_colmajor(N, N, w.dtype, dev); H.copy_(w.H)
+    V = W.empty_colmajor(N, n, w.dtype, dev); V.copy_(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(N, n, w.dtype), dtype=torch.uint8, device=dev)
+    ws.fill_(0xFF)
+    pkg.chase_filter_ws(H, V, w.degrees, w.a, w.b, w.lambda1, ws)
+    torch.cuda.synchronize()
+    ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), w.degrees.numpy(), w.a, w.b, w.lambda1)
+    got = V.cpu().numpy()
+    assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 1e-12
+    assert torch.equal(H.cpu(), w.H)

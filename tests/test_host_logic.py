@@ -144,10 +144,15 @@ def test_step_plan_covers_every_tile_slab_exactly_once(dtype, bn, quarter, bk):
                 T, D, G, KT = tm * tn, pl["dp_tiles"], pl["sk_ctas"], pl["slabs_per_tile"]
                 assert 0 <= D <= T and 0 <= G <= min(sms, 160)
                 skb = pl["sk_begin"]
+                grid, rounds = pl["grid"], pl["dp_rounds"]
                 if G == 0:
-                    assert D == T
+                    assert D == T and grid == T and rounds == 1     # one CTA per tile
                     continue
-                assert D % sms == 0                                # the data-parallel part is whole waves
+                # whole tiles: CTA b owns r * grid + b < D for r < rounds -- every tile below D exactly once;
+                # default plan: persistent CTAs (lock-step), stream-K ranges on the same CTAs
+                first = pl["sk_first"]
+                assert (rounds, first, grid) == ((D // sms, 0, sms) if D > 0 else (0, 0, G))
+                assert D % sms == 0
                 assert len(skb) == G + 1 and skb[0] == 0 and skb[-1] == (T - D) * KT
                 assert np.all(np.diff(skb) >= 0)
 
@@ -164,34 +169,36 @@ def test_step_plan_balances_the_benchmark_configs():
         warps_n, group_n = (2, 16) if cplx else (4, 12)
         w, tm, tn, KT = pl["tile_width"], pl["tiles_m"], pl["tiles_n"], pl["slabs_per_tile"]
 
-        def quarters(t):                                          # cost of one slab of raster tile t
-            per_group = group_n * tm
-            grp = t // per_group
-            first = grp * group_n
-            gn = min(group_n, tn - first)
-            col = first + (t - grp * per_group) % gn
+        def quarters(t, ragged_last):                             # cost of one slab of raster tile t
+            body_n = tn - 1 if ragged_last else tn                # lock-step plans: the ragged tile column comes last
+            if t >= body_n * tm:
+                col = body_n
+            else:
+                per_group = group_n * tm
+                grp = t // per_group
+                first = grp * group_n
+                gn = min(group_n, body_n - first)
+                col = first + (t - grp * per_group) % gn
             v = min(w, n - col * w)
             return -(-(-(-v // 8)) // warps_n)
 
-        heap = [0.0] * sms
-        total = 0.0
-        for t in range(pl["dp_tiles"]):
-            f = heapq.heappop(heap)
-            heapq.heappush(heap, f + quarters(t) * KT)
-            total += quarters(t) * KT
-        end = max(heap) if pl["sk_ctas"] == 0 else 0.0
+        grid, rounds = pl["grid"], pl["dp_rounds"]
+        busy = [0.0] * grid                                       # persistent CTAs, one per SM
+        for r in range(rounds):
+            for b in range(grid):
+                t = r * grid + b
+                if t < pl["dp_tiles"]:
+                    busy[b] += quarters(t, rounds > 0) * KT
         skb = pl["sk_begin"]
         for g in range(pl["sk_ctas"]):
-            f = heapq.heappop(heap)
-            cost, s = 0.0, int(skb[g])
+            s = int(skb[g])
             while s < skb[g + 1]:
                 t = pl["dp_tiles"] + s // KT
                 take = min(int(skb[g + 1]) - s, KT - s % KT)
-                cost += take * quarters(t)
+                busy[g] += take * quarters(t, rounds > 0)
                 s += take
-            total += cost
-            end = max(end, f + cost)
-        return end, total / sms
+        assert grid <= sms or pl["sk_ctas"] == 0
+        return max(busy), sum(busy) / sms
 
     for N, n, dtype, slack in ((512, 60, torch.complex128, 1.10), (4096, 256, torch.complex128, 1.01),
                                (4096, 37, torch.complex128, 1.03), (40000, 2000, torch.complex128, 1.002),
