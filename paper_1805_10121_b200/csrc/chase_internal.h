@@ -100,6 +100,7 @@ struct Tf32Plan {
     void *buf[2];
     void *sync_ctr;                             // 4-byte counter of the producers' soft grid barrier
     int pair;                                   // 1: CTA-pair kernel (cta_group::2, 256-row tiles), 0: single-CTA kernel
+    int mixed;                                  // 1: TF32 hi*hi + one BF16 MMA for both cross terms, 0: classic 3xTF32
 };
 bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);
 int tf32_vector_blocks(chase_dtype_t dtype);    // vector-sized blocks in the workspace besides H_lo

@@ -102,6 +102,16 @@ __device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint6
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
         ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate) : "memory");
 }
+// kind::f16 with BF16 operands (a_format = b_format = 1), fp32 accumulate: same tile shape, K = 16 per instruction
+constexpr uint32_t kInstrDescBf16 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) |
+                                    ((uint32_t)(TM >> 4) << 24);
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDescBf16), "r"(accumulate) : "memory");
+}
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
 }
@@ -132,6 +142,28 @@ __device__ __forceinline__ void sts128(uint32_t addr, float4 v) {
 __device__ __forceinline__ float4 split_lo(float4 v) {
     return make_float4(v.x - tf32_hi(v.x), v.y - tf32_hi(v.y), v.z - tf32_hi(v.z), v.w - tf32_hi(v.w));
 }
+// Mixed scheme (DESIGN.md 6.4 "TF32 + BF16 cross terms"): the two small products hi*lo + lo*hi of a k-slice are
+// ONE kind::f16 MMA over a doubled K: the 16-byte chunk that holds the fp32 values x0..x3 (k .. k+3) becomes the
+// 16-byte chunk of 8 BF16 values [x0 x1 x2 x3 | l0 l1 l2 l3] for A and [l0 l1 l2 l3 | x0 x1 x2 x3] for B
+// (l = x - tf32_hi(x), both rounded to nearest BF16), so slot s of A meets slot s of B: sum_k xA lB + lA xB.
+// Element-wise per chunk, hence at the same (swizzled) position as the raw chunk.
+__device__ __forceinline__ uint32_t bf16x2(float lo_elem, float hi_elem) {
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_elem), "f"(lo_elem));   // first source -> upper half
+    return r;
+}
+template <bool B_SIDE>
+__device__ __forceinline__ float4 pack_pair(float4 v) {
+    const float4 l = make_float4(v.x - tf32_hi(v.x), v.y - tf32_hi(v.y), v.z - tf32_hi(v.z), v.w - tf32_hi(v.w));
+    const float x01 = __uint_as_float(bf16x2(v.x, v.y)), x23 = __uint_as_float(bf16x2(v.z, v.w));
+    const float l01 = __uint_as_float(bf16x2(l.x, l.y)), l23 = __uint_as_float(bf16x2(l.z, l.w));
+    return B_SIDE ? make_float4(l01, l23, x01, x23) : make_float4(x01, x23, l01, l23);
+}
+// the second tile of an operand: its lo part (3xTF32) or its BF16 pair tile (mixed scheme)
+template <bool B_SIDE>
+__device__ __forceinline__ float4 second_tile(float4 v, int mixed) {
+    return mixed ? pack_pair<B_SIDE>(v) : split_lo(v);
+}
 __device__ __forceinline__ float4 rot_mi(float4 v) { return make_float4(v.y, -v.x, v.w, -v.z); }   // -i (x + iy) pairs
 
 
@@ -147,6 +179,7 @@ struct Tf32Params {
     const double *c_col;
     int use_beta;
     unsigned *sync_ctr;                 // soft grid barrier counter (zeroed before the launch) or nullptr
+    int mixed;                          // 1: hi*hi in TF32 + one BF16 MMA for the cross terms; 0: classic 3xTF32
 };
 
 #ifndef TF32_SYNC_STAGES
@@ -284,9 +317,13 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                             const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
                             const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
                             const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
-                            umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
-                            umma_tf32(d, al, bh, 1u);                 // lo * hi
-                            umma_tf32(d, ah, bh, 1u);                 // hi * hi
+                            if (p.mixed) {
+                                umma_bf16(d, al, bl, first ? 0u : 1u);    // x_b * lo_b + lo_b * x_b (pair tiles, K = 16)
+                            } else {
+                                umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
+                                umma_tf32(d, al, bh, 1u);                 // lo * hi
+                            }
+                            umma_tf32(d, ah, bh, 1u);                     // hi * hi
                             first = false;
                         }
                         umma_commit(bar_base + 8 * (STAGES + s));   // frees the smem stage when these MMAs retire
@@ -319,14 +356,15 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 #pragma unroll
                         for (int i = 0; i < NB; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
+                        for (int i = 0; i < NA; ++i)
+                            sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, second_tile<false>(va[i], p.mixed));
 #pragma unroll
                         for (int i = 0; i < NB; ++i) {
                             const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                            const float4 lo = split_lo(vb[i]);
-                            sts128(sb_lo + off, lo);
-                            sts128(sb_hi + B_BYTES / 2 + off, rot_mi(vb[i]));
-                            sts128(sb_lo + B_BYTES / 2 + off, rot_mi(lo));
+                            const float4 r = rot_mi(vb[i]);            // lo(-iX) = -i lo(X): the split is element-wise
+                            sts128(sb_lo + off, second_tile<true>(vb[i], p.mixed));
+                            sts128(sb_hi + B_BYTES / 2 + off, r);
+                            sts128(sb_lo + B_BYTES / 2 + off, second_tile<true>(r, p.mixed));
                         }
                     } else {
                         constexpr int NB = B_BYTES / 16 / CT;
@@ -334,14 +372,16 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 #pragma unroll
                         for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
 #pragma unroll
-                        for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
+                        for (int i = 0; i < NA; ++i)
+                            sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, second_tile<false>(va[i], p.mixed));
 #pragma unroll
-                        for (int i = 0; i < NB / 2; ++i) sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, split_lo(vb[i]));
+                        for (int i = 0; i < NB / 2; ++i)
+                            sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, second_tile<true>(vb[i], p.mixed));
 #pragma unroll
                         for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + (i + NB / 2) * CT) * 16);
 #pragma unroll
                         for (int i = 0; i < NB / 2; ++i)
-                            sts128(sb_lo + (uint32_t)(ct + (i + NB / 2) * CT) * 16, split_lo(vb[i]));
+                            sts128(sb_lo + (uint32_t)(ct + (i + NB / 2) * CT) * 16, second_tile<true>(vb[i], p.mixed));
                     }
                 }
                 // generic-proxy writes -> visible to the tensor core's async-proxy reads
@@ -420,6 +460,21 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 // multicast to both); the barriers that gate the single MMA issuer (CTA 0) -- "converted" and
 // "accumulator drained" -- live in CTA 0 and take remote arrivals from CTA 1 (mapa + cluster-scope
 // release / acquire).
+// Thread layout of the pair kernel (4 warpgroups, registers rebalanced with setmaxnreg): warpgroup 0 = TMA producer,
+// MMA issuer, two idle warps (40 registers); warpgroups 1-2 = accumulator / epilogue warps (184); warpgroup 3 =
+// converter warps (104).  The converters form kConvGroups2 groups of kConvWpg2 warps; group g derives the second
+// tiles of the stages it % kConvGroups2 == g, so the fixed latencies of consecutive stages (barrier wait, LDS
+// round trip, fence.proxy.async) overlap.  Measured: with two converter warps that serial chain,
+// not the tensor core, set the stage time (1320 clk against an MMA floor of 512-768).
+#ifndef TF32_CONV_GROUPS
+#define TF32_CONV_GROUPS 2
+#endif
+constexpr int kConvWarps2 = 4;
+constexpr int kConvGroups2 = TF32_CONV_GROUPS;
+constexpr int kConvWpg2 = kConvWarps2 / kConvGroups2;
+constexpr int kFirstConvWarp2 = kFirstAccWarp + kAccWarps;     // 12
+constexpr int kThreads2 = (kFirstConvWarp2 + kConvWarps2) * 32;   // 512
+static_assert(kConvGroups2 * kConvWpg2 == kConvWarps2, "converter groups must tile the converter warps");
 constexpr int STAGES2 = 6;
 constexpr int BH = TN / 2;                       // real B columns held by one CTA of a pair
 constexpr int B2_BYTES = BH * KS * 4;            // 8 KB
@@ -457,6 +512,15 @@ __device__ __forceinline__ void umma_tf32_pair(uint32_t tmem_d, uint64_t adesc, 
         "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
         ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDesc2), "r"(accumulate) : "memory");
 }
+constexpr uint32_t kInstrDescBf16Pair = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) |
+                                        ((uint32_t)((2 * TM) >> 4) << 24);
+__device__ __forceinline__ void umma_bf16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n.reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}\n"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDescBf16Pair), "r"(accumulate) : "memory");
+}
 // arrives (once the MMAs issued so far have retired) on the barrier at this offset in BOTH CTAs of the pair
 __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
     asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
@@ -464,7 +528,7 @@ __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
 }
 
 template <bool CPLX>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads2, 1)
 step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
                       const Tf32Params p) {
     constexpr int COLS = CPLX ? TN / 2 : TN;      // (complex or real) columns per pair tile
@@ -488,7 +552,7 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         for (int s = 0; s < STAGES2; ++s) {
             mbar_init(bar_base + 8 * s, 1);                       // full: this CTA's producer (expect_tx)
             mbar_init(bar_base + 8 * (STAGES2 + s), 1);           // empty: one multicast tcgen05.commit
-            mbar_init(bar_conv + 8 * s, 2 * kConvWarps);          // conv (used in CTA 0): converter warps of both CTAs
+            mbar_init(bar_conv + 8 * s, 2 * kConvWpg2);           // conv (used in CTA 0): one converter group of both CTAs
         }
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_tfull + 8 * b, 1);                      // chunk accumulator complete (multicast commit)
@@ -505,6 +569,8 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     uint32_t tmem_base;
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
+
+    if (warp < kFirstAccWarp) asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
 
     if (warp == 0) {
         // ------------------------------------------------------------------ TMA producer (both CTAs)
@@ -563,9 +629,13 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                             const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
                             const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
                             const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
-                            umma_tf32_pair(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
-                            umma_tf32_pair(d, al, bh, 1u);                 // lo * hi
-                            umma_tf32_pair(d, ah, bh, 1u);                 // hi * hi
+                            if (p.mixed) {
+                                umma_bf16_pair(d, al, bl, first ? 0u : 1u);    // x_b * lo_b + lo_b * x_b (pair tiles, K = 16)
+                            } else {
+                                umma_tf32_pair(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
+                                umma_tf32_pair(d, al, bh, 1u);                 // lo * hi
+                            }
+                            umma_tf32_pair(d, ah, bh, 1u);                     // hi * hi
                             first = false;
                         }
                         umma_commit_pair(bar_base + 8 * (STAGES2 + s));   // frees the stage in both CTAs when these MMAs retire
@@ -574,46 +644,58 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 }
             }
         }
-    } else if (warp < 2 + kConvWarps) {
+    } else if (warp >= kFirstConvWarp2) {
         // ------------------------------------------------------------------ converter warps (both CTAs)
-        constexpr int CT = kConvWarps * 32;
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        constexpr int CT = kConvWpg2 * 32;                       // threads that share one stage
         constexpr int NA = A_BYTES / 16 / CT, NBV = B2_BYTES / 16 / CT;
-        const int ct = threadIdx.x - 64;
+        constexpr int BATCH = NA < 8 ? NA : 8;                   // 16-byte chunks of A (and of B) in flight per thread
+        const int grp = (warp - kFirstConvWarp2) / kConvWpg2;
+        const int ct = ((warp - kFirstConvWarp2) % kConvWpg2) * 32 + lane;
         const uint32_t leader_conv = mapa_shared(bar_conv, 0);
         unsigned it = 0;
         for (int tile = pair; tile < total_tiles; tile += npairs) {
             for (int kt = 0; kt < KT; ++kt, ++it) {
+                if ((int)(it % kConvGroups2) != grp) continue;
                 const int s = it % STAGES2;
                 mbar_wait(bar_base + 8 * s, (it / STAGES2) & 1);
                 const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sa_lo = sa_hi + A_BYTES;
                 const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B2_BYTES;
-                float4 va[NA], vb[NBV];
 #pragma unroll
-                for (int i = 0; i < NA; ++i) va[i] = lds128(sa_hi + (uint32_t)(ct + i * CT) * 16);
+                for (int b0 = 0; b0 < NA; b0 += BATCH) {
+                    float4 va[BATCH], vb[BATCH];
 #pragma unroll
-                for (int i = 0; i < NBV; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
+                    for (int i = 0; i < BATCH; ++i) va[i] = lds128(sa_hi + (uint32_t)(ct + (b0 + i) * CT) * 16);
 #pragma unroll
-                for (int i = 0; i < NA; ++i) sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, split_lo(va[i]));
-                if (CPLX && rank == 1) {
-                    // this CTA supplies -iX: rotate the raw tile in place (a thread rewrites the chunk it read)
+                    for (int i = 0; i < BATCH; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + (b0 + i) * CT) * 16);
 #pragma unroll
-                    for (int i = 0; i < NBV; ++i) {
-                        const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                        sts128(sb_hi + off, rot_mi(vb[i]));
-                        sts128(sb_lo + off, rot_mi(split_lo(vb[i])));
+                    for (int i = 0; i < BATCH; ++i)
+                        sts128(sa_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<false>(va[i], p.mixed));
+                    if (CPLX && rank == 1) {
+                        // this CTA supplies -iX: rotate the raw tile in place (a thread rewrites the chunk it read)
+#pragma unroll
+                        for (int i = 0; i < BATCH; ++i) {
+                            const uint32_t off = (uint32_t)(ct + (b0 + i) * CT) * 16;
+                            const float4 r = rot_mi(vb[i]);
+                            sts128(sb_hi + off, r);
+                            sts128(sb_lo + off, second_tile<true>(r, p.mixed));
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < BATCH; ++i)
+                            sts128(sb_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<true>(vb[i], p.mixed));
                     }
-                } else {
-#pragma unroll
-                    for (int i = 0; i < NBV; ++i) sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, split_lo(vb[i]));
                 }
+                static_assert(NA == NBV && NA % BATCH == 0, "A and B halves of a stage have the same size");
                 // generic-proxy writes -> visible to the tensor core's async-proxy reads
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
                 if (lane == 0) mbar_arrive_cluster(leader_conv + 8 * s);
             }
         }
-    } else if (warp >= kFirstAccWarp) {
+    } else if (warp >= kFirstAccWarp && warp < kFirstConvWarp2) {
         // ------------------------------------------------------------------ accumulator / epilogue warps (both CTAs)
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
         const int quarter = warp & 3;
         const int half = (warp - kFirstAccWarp) >> 2;
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
@@ -743,6 +825,7 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     p.c_col = c_col;
     p.use_beta = use_beta;
     p.sync_ctr = (unsigned *)plan->sync_ctr;
+    p.mixed = plan->mixed;
     const int total_tiles = p.tiles_m * p.tiles_n;
     if (p.sync_ctr) {
         cudaError_t e = cudaMemsetAsync(p.sync_ctr, 0, sizeof(unsigned), stream);
@@ -750,7 +833,7 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     }
     if (pair) {   // persistent CTA pairs: one cluster of 2 per TPC
         const int grid = 2 * std::min(total_tiles, std::max(1, sm_count() / 2));
-        step_tf32_pair_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM2_TOTAL, stream>>>(
+        step_tf32_pair_kernel<CPLX><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
             *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
         count_launch();
         return cudaGetLastError();
@@ -787,6 +870,9 @@ cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H,
     // CTA pairs (cta_group::2) unless CHASE_TF32_PAIR=0 asks for the single-CTA kernel (experiments / fallback)
     const char *pair_env = std::getenv("CHASE_TF32_PAIR");
     plan->pair = !(pair_env && pair_env[0] == '0');
+    // cross terms hi*lo + lo*hi as ONE BF16 MMA (2 MMA units per product) unless CHASE_TF32_MIXED=0 (classic 3xTF32)
+    const char *mixed_env = std::getenv("CHASE_TF32_MIXED");
+    plan->mixed = !(mixed_env && mixed_env[0] == '0');
     cudaError_t e;
     if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A, H, KF, N, TM)) != cudaSuccess) return e;
     const int b_box = plan->pair ? TN / 2 : (cplx ? TN / 2 : TN);      // B columns one TMA box brings
