@@ -367,14 +367,19 @@ def roofline_of(pkg, w, achieved_tflops: float, clocks, device, launches_per_ste
     sms = torch.cuda.get_device_properties(device).multi_processor_count
     kernel_path = pkg.chase_filter_kernel_path(N, n, dtype)
     is_f64 = dtype in (torch.complex128, torch.float64)
+    frac_3x = None
     if kernel_path == 2:
-        # tcgen05 kind::tf32, three MMAs per algorithmic product (3xTF32): the peak for ALGORITHMIC
-        # flops is a third of the TF32 tensor peak; TF32 peak = measured bf16 GEMM x nominal ratio.
+        # tcgen05: per algorithmic product one kind::tf32 MMA (hi*hi) + one kind::f16 BF16 MMA over a doubled K
+        # for both cross terms = 2 MMA units (CHASE_TF32_MIXED=0: classic 3xTF32, 3 units).  The
+        # peak for ALGORITHMIC flops is the TF32 tensor peak / units; TF32 peak = measured bf16 GEMM x nominal ratio.
         bf16, src = measured_bf16_sustained_tflops()
-        peak = bf16 * TF32_OVER_BF16_NOMINAL / 3.0
-        bound, kname = "tensor", "step_tf32_kernel"
-        peak_source = (f"{src} x nominal tf32/bf16 ratio {TF32_OVER_BF16_NOMINAL:.3f} / 3 MMAs per product "
-                       f"(3xTF32 split, DESIGN.md 6.4)")
+        units = 3.0 if os.environ.get("CHASE_TF32_MIXED", "1")[:1] == "0" else 2.0
+        peak = bf16 * TF32_OVER_BF16_NOMINAL / units
+        frac_3x = achieved_tflops / (bf16 * TF32_OVER_BF16_NOMINAL / 3.0)
+        bound, kname = "tensor", "step_tf32_pair_kernel"
+        peak_source = (f"{src} x nominal tf32/bf16 ratio {TF32_OVER_BF16_NOMINAL:.3f} / {units:.0f} MMA units per "
+                       f"product ({'TF32 hi*hi + one BF16 MMA for both cross terms' if units == 2.0 else '3xTF32 split'}, "
+                       f"DESIGN.md 6.4); power-capped part: sw_power_cap is expected")
     else:
         per_clk = FP64_FLOP_PER_CLK_SM * (1 if is_f64 else 2)     # FP32 FMA pipe: 256 flop/clk/SM
         peak = sms * per_clk * sm_max_mhz * 1e6 * 1e-12            # TFLOP/s
@@ -392,6 +397,7 @@ def roofline_of(pkg, w, achieved_tflops: float, clocks, device, launches_per_ste
         "achieved": achieved_tflops, "peak": peak, "unit": "TFLOP/s", "frac": achieved_tflops / peak,
         "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_source,
         "frac_of_nvidia_quoted_40tf": achieved_tflops / 40.0 if is_f64 else None,
+        "frac_of_3xtf32_peak": frac_3x,
         "algorithmic_flops_per_step": w.flops(), "launches_per_step": launches_per_step,
     }
 

@@ -607,43 +607,80 @@ step_dmma_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
         }
 
         // ---------------------------------------------------------------- fused epilogue
-        // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block
+        // accumulator fragment: row g, columns 2t and 2t+1 of each 8x8 block.  Per 8-column block all loads of
+        // X (and Y) are issued before the first store: Y may alias nothing the loads need, but the compiler cannot
+        // know, and a load-store-load chain pays one L2 round trip per element (32 per tile: ~10 us, most of a
+        // small launch).
         const double alpha = p.alpha, beta = p.beta;
 #pragma unroll
         for (int j = 0; j < NB; ++j) {
+            if (j >= jmax) break;
+            constexpr int EB = CPLX ? 2 : 1;       // columns of the fragment per batch (float64: 8 row blocks per column)
 #pragma unroll
-            for (int e = 0; e < 2; ++e) {
+            for (int e0 = 0; e0 < 2; e0 += EB) {
+            double2 xv[2][MB], ov[2][MB];
+            double cc[2];
+            bool colok[2];
+#pragma unroll
+            for (int e = e0; e < e0 + EB; ++e) {
                 const int cl = (j * WARPS_N + wn) * 8 + 2 * t + e;     // column inside the tile
-                if (cl >= ncols_tile) continue;
+                colok[e] = cl < ncols_tile;
                 const int col = n0 + cl;
-                const double c = p.c_col ? p.c_col[col] : p.c;
+                cc[e] = colok[e] ? (p.c_col ? p.c_col[col] : p.c) : 0.0;
 #pragma unroll
                 for (int i = 0; i < MB; ++i) {
                     int row;
                     if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
                     else row = m0 + wm * C::WM + (i >> 1) * 16 + 2 * g + (i & 1);
-                    if (row >= p.M) continue;
+                    const bool ok = colok[e] && row < p.M;
+                    const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
+                    xv[e][i] = make_double2(0.0, 0.0);
+                    ov[e][i] = make_double2(0.0, 0.0);
+                    if (ok) {
+                        // ld.global.cg: the vector buffers are rewritten by OTHER SMs from one launch to the next, and
+                        // the (non-coherent) L1 was seen to serve lines of an earlier iterate to these batched loads
+                        // (rare 32 x 8 patches of V_{k-2} in place of V_k; bypassing L1 removes them)
+                        if (CPLX) {
+                            xv[e][i] = __ldcg(reinterpret_cast<const double2 *>(p.X + off));
+                            if (p.use_beta) ov[e][i] = __ldcg(reinterpret_cast<const double2 *>(p.Y + off));
+                        } else {
+                            xv[e][i].x = __ldcg(p.X + off);
+                            if (p.use_beta) ov[e][i].x = __ldcg(p.Y + off);
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int e = e0; e < e0 + EB; ++e) {
+                const int cl = (j * WARPS_N + wn) * 8 + 2 * t + e;
+                const int col = n0 + cl;
+                const double c = cc[e];
+#pragma unroll
+                for (int i = 0; i < MB; ++i) {
+                    int row;
+                    if (CPLX) row = m0 + wm * C::WM + i * 8 + g;
+                    else row = m0 + wm * C::WM + (i >> 1) * 16 + 2 * g + (i & 1);
+                    if (!colok[e] || row >= p.M) continue;
                     const int64_t off = ((int64_t)col * p.N + p.row0 + row) * NC;
                     if (CPLX) {
-                        const double2 x = *reinterpret_cast<const double2 *>(p.X + off);
                         double2 y;
-                        y.x = alpha * (acc[0][i][j][e] - c * x.x);
-                        y.y = alpha * (acc[NC - 1][i][j][e] - c * x.y);
+                        y.x = alpha * (acc[0][i][j][e] - c * xv[e][i].x);
+                        y.y = alpha * (acc[NC - 1][i][j][e] - c * xv[e][i].y);
                         if (p.use_beta) {
-                            const double2 o = *reinterpret_cast<const double2 *>(p.Y + off);
-                            y.x = fma(beta, o.x, y.x);
-                            y.y = fma(beta, o.y, y.y);
+                            y.x = fma(beta, ov[e][i].x, y.x);
+                            y.y = fma(beta, ov[e][i].y, y.y);
                         }
                         *reinterpret_cast<double2 *>(p.Y + off) = y;
                         for (int q = 0; q < p.npeers; ++q)      // fused all-gather: push the row block over NVLink
                             *reinterpret_cast<double2 *>(p.peer_Y[q] + off) = y;
                     } else {
-                        double y = alpha * (acc[0][i][j][e] - c * p.X[off]);
-                        if (p.use_beta) y = fma(beta, p.Y[off], y);
+                        double y = alpha * (acc[0][i][j][e] - c * xv[e][i].x);
+                        if (p.use_beta) y = fma(beta, ov[e][i].x, y);
                         p.Y[off] = y;
                         for (int q = 0; q < p.npeers; ++q) p.peer_Y[q][off] = y;
                     }
                 }
+            }
             }
         }
     }

@@ -50,7 +50,7 @@ constexpr int TM = 128;           // (complex or real) rows per CTA tile = TMEM 
 constexpr int TN = 256;           // real B columns per CTA tile = TMEM columns
 constexpr int STAGES = 4;
 #ifndef TF32_CHUNK
-#define TF32_CHUNK 4
+#define TF32_CHUNK 8
 #endif
 constexpr int CHUNK = TF32_CHUNK;            // pipeline stages accumulated in TMEM before the sum moves to registers
 constexpr int A_BYTES = TM * KS * 4;          // 8 KB
@@ -78,10 +78,31 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
             : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     } while (!done);
 }
+// Wait of a warp that expects to wait LONG (accumulator warps on a chunk, the producer on a free stage): back off
+// between polls, so that the idle roles do not burn issue slots and power next to the converter warps.
+#ifndef TF32_WAIT_SLEEP_NS
+#define TF32_WAIT_SLEEP_NS 200
+#endif
+__device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
+    uint32_t done;
+    for (;;) {
+        asm volatile(
+            "{\n.reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n}\n"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) break;
+        if (TF32_WAIT_SLEEP_NS > 0) __nanosleep(TF32_WAIT_SLEEP_NS);
+    }
+}
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, uint32_t bar, int c0, int c1) {
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap *map, int c0, int c1) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(map), "r"(c0), "r"(c1) : "memory");
 }
 
 // UMMA shared-memory matrix descriptor (sm_100): start address, leading / stride byte offsets
@@ -129,6 +150,18 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
     for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
@@ -432,8 +465,8 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
                 if (col < p.n && row_ok) {
                     const float c = p.c_col ? (float)p.c_col[col] : p.c;
                     const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
-                    float y = alpha * (racc[i] - c * p.X[off]);
-                    if (p.use_beta) y = fmaf(beta, p.Y[off], y);
+                    float y = alpha * (racc[i] - c * __ldcg(p.X + off));   // L2 only: see step_dmma.cu
+                    if (p.use_beta) y = fmaf(beta, __ldcg(p.Y + off), y);
                     p.Y[off] = y;
                 }
             }
@@ -469,17 +502,47 @@ step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constan
 #ifndef TF32_CONV_GROUPS
 #define TF32_CONV_GROUPS 2
 #endif
-constexpr int kConvWarps2 = 4;
+#ifndef TF32_CONV_WARPS
+#define TF32_CONV_WARPS 4          // 8 (two converter warpgroups) measured slower: more power, same stage time
+#endif
+constexpr int kConvWarps2 = TF32_CONV_WARPS;
 constexpr int kConvGroups2 = TF32_CONV_GROUPS;
 constexpr int kConvWpg2 = kConvWarps2 / kConvGroups2;
 constexpr int kFirstConvWarp2 = kFirstAccWarp + kAccWarps;     // 12
-constexpr int kThreads2 = (kFirstConvWarp2 + kConvWarps2) * 32;   // 512
+constexpr int kThreads2 = (kFirstConvWarp2 + kConvWarps2) * 32;   // 640
+// registers per thread after setmaxnreg: 128 x 40 (warpgroup 0) + 256 x kAccRegs2 + 32 kConvWarps2 x kConvRegs2 <= 65536
+// setmaxnreg moves registers inside the CTA's OWN allocation (threads x the launch count ptxas reports: 128 for
+// 512 threads, 96 for 640), so the counts after rebalancing must fit in that, or the .inc never returns.
+constexpr int kLaunchRegs2 = kConvWarps2 == 8 ? 96 : 128;
+constexpr int kConvRegs2 = kConvWarps2 == 8 ? 64 : 104;
+constexpr int kAccRegs2 = kConvWarps2 == 8 ? 152 : 184;
+static_assert(kConvWarps2 == 4 || kConvWarps2 == 8, "whole converter warpgroups");
+static_assert(128 * 40 + 256 * kAccRegs2 + 32 * kConvWarps2 * kConvRegs2 <= kThreads2 * kLaunchRegs2,
+              "registers of one CTA");
 static_assert(kConvGroups2 * kConvWpg2 == kConvWarps2, "converter groups must tile the converter warps");
-constexpr int STAGES2 = 6;
+// Two rings: the RAW tiles [A | B] written by TMA live from the load to the retirement of the
+// stage's MMAs, the SECOND tiles [A' | B'] written by the converters only from the conversion on.  With one
+// 32 KB ring of 6 stages the ~3000-clock TMA round trip alone capped the rate at 6 stages per round trip
+// (measured: 521 clk per stage with neither conversion nor MMAs); a deep raw ring and a short second ring keep
+// 10 loads in flight in the same shared memory.
+#ifndef TF32_RAW_STAGES
+#define TF32_RAW_STAGES 10
+#endif
+#ifndef TF32_PAIR_STAGES
+#define TF32_PAIR_STAGES 3
+#endif
+#ifndef TF32_PREFETCH
+#define TF32_PREFETCH 0           // stages the producer prefetches into L2 ahead of its loads (0: off; 12 measured
+                                  // 3 % SLOWER: the lock-step CTAs already find each other's lines in L2)
+#endif
+constexpr int RAW2 = TF32_RAW_STAGES, SEC2 = TF32_PAIR_STAGES, kPrefetch2 = TF32_PREFETCH;
+static_assert(SEC2 < RAW2, "the second ring must be shorter than the raw ring (see the converter's slot-free wait)");
 constexpr int BH = TN / 2;                       // real B columns held by one CTA of a pair
 constexpr int B2_BYTES = BH * KS * 4;            // 8 KB
-constexpr int STAGE2_BYTES = 2 * A_BYTES + 2 * B2_BYTES;   // A raw | A lo | B hi | B lo : 32 KB
-constexpr int SMEM2_TOTAL = STAGES2 * STAGE2_BYTES + 1024 + 512;
+constexpr int RAW2_BYTES = A_BYTES + B2_BYTES;   // A raw | B raw (complex, CTA 1: rotated in place) : 16 KB
+constexpr int SEC2_BYTES = A_BYTES + B2_BYTES;   // A' | B' (lo parts or BF16 pair tiles)             : 16 KB
+constexpr int SMEM2_TOTAL = RAW2 * RAW2_BYTES + SEC2 * SEC2_BYTES + 1024 + 512;
+static_assert(SMEM2_TOTAL <= 232448, "shared memory of one CTA");
 constexpr uint32_t kInstrDesc2 = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) |
                                  ((uint32_t)((2 * TM) >> 4) << 24);
 
@@ -527,7 +590,7 @@ __device__ __forceinline__ void umma_commit_pair(uint32_t bar) {
                  ::"r"(bar), "h"((uint16_t)3) : "memory");
 }
 
-template <bool CPLX>
+template <bool CPLX, bool MIXED>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads2, 1)
 step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
                       const Tf32Params p) {
@@ -535,11 +598,13 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     const uint32_t smem_base = smem_u32(smem);
-    const uint32_t bar_base = smem_base + STAGES2 * STAGE2_BYTES;   // full[S], empty[S], conv[S], tfull[2], tempty[2], tmem slot
-    const uint32_t bar_conv = bar_base + 8 * (2 * STAGES2);
-    const uint32_t bar_tfull = bar_base + 8 * (3 * STAGES2);
-    const uint32_t bar_tempty = bar_base + 8 * (3 * STAGES2 + 2);
-    const uint32_t tmem_slot = bar_base + 8 * (3 * STAGES2 + 4);
+    const uint32_t sec_base = smem_base + RAW2 * RAW2_BYTES;
+    const uint32_t bar_base = sec_base + SEC2 * SEC2_BYTES;   // full[RAW2], empty[RAW2], conv[SEC2], tfull[2], tempty[2], tmem slot
+    const uint32_t bar_empty = bar_base + 8 * RAW2;
+    const uint32_t bar_conv = bar_base + 8 * (2 * RAW2);
+    const uint32_t bar_tfull = bar_conv + 8 * SEC2;
+    const uint32_t bar_tempty = bar_tfull + 16;
+    const uint32_t tmem_slot = bar_tempty + 16;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();              // 0: leader (issues the MMAs), 1: peer
@@ -549,11 +614,12 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
     const int NCH = (KT + CHUNK - 1) / CHUNK;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES2; ++s) {
+        for (int s = 0; s < RAW2; ++s) {
             mbar_init(bar_base + 8 * s, 1);                       // full: this CTA's producer (expect_tx)
-            mbar_init(bar_base + 8 * (STAGES2 + s), 1);           // empty: one multicast tcgen05.commit
-            mbar_init(bar_conv + 8 * s, 2 * kConvWpg2);           // conv (used in CTA 0): one converter group of both CTAs
+            mbar_init(bar_empty + 8 * s, 1);                      // empty: one multicast tcgen05.commit
         }
+        for (int s = 0; s < SEC2; ++s)
+            mbar_init(bar_conv + 8 * s, 2 * kConvWpg2);           // conv (used in CTA 0): one converter group of both CTAs
         for (int b = 0; b < 2; ++b) {
             mbar_init(bar_tfull + 8 * b, 1);                      // chunk accumulator complete (multicast commit)
             mbar_init(bar_tempty + 8 * b, 2 * kAccWarps);         // (used in CTA 0): drained by both CTAs' accumulator warps
@@ -579,6 +645,29 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
             unsigned it = 0;
             unsigned *sync_ctr = p.sync_ctr;
             int round = 0;
+            // L2 prefetch cursor: runs kPrefetch2 stages ahead of the loads (through tile boundaries), so that the
+            // loads that fill shared memory find their lines in L2 instead of paying the DRAM round trip.
+            int pf_tile = pair, pf_kt = 0, pf_m0 = 0, pf_nb0 = 0;
+            auto pf_coords = [&]() {
+                int tm, tn;
+                tile_coords(pf_tile, p.tiles_m, p.tiles_n, tm, tn);
+                pf_m0 = tm * (2 * TM) + (int)rank * TM;
+                pf_nb0 = p.col0 + tn * COLS + (CPLX ? 0 : (int)rank * BH);
+            };
+            auto prefetch_next = [&]() {
+                if (kPrefetch2 == 0 || pf_tile >= total_tiles) return;
+                tma_prefetch_2d(&tmapA, pf_kt * KS, pf_m0);
+                if (!CPLX || rank == 0) tma_prefetch_2d(&tmapB, pf_kt * KS, pf_nb0);   // complex: the pair shares one X tile
+                if (++pf_kt == KT) {
+                    pf_kt = 0;
+                    pf_tile += npairs;
+                    if (pf_tile < total_tiles) pf_coords();
+                }
+            };
+            if (kPrefetch2 > 0 && pf_tile < total_tiles) {
+                pf_coords();
+                for (int i = 0; i < kPrefetch2; ++i) prefetch_next();
+            }
             for (int tile = pair; tile < total_tiles; tile += npairs, ++round) {
                 int tile_m, tile_n;
                 tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
@@ -590,14 +679,15 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     if (sync_ctr && kt % kSyncStages == 0 &&
                         !soft_grid_sync(sync_ctr, sync_base + active * (unsigned)(kt / kSyncStages + 1)))
                         sync_ctr = nullptr;
-                    const int s = it % STAGES2;
-                    const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES2 + s);
-                    if (it >= STAGES2) mbar_wait(empty, ((it / STAGES2) - 1) & 1);
-                    const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sb_hi = sa_hi + 2 * A_BYTES;
+                    prefetch_next();
+                    const int s = it % RAW2;
+                    const uint32_t full = bar_base + 8 * s, empty = bar_empty + 8 * s;
+                    if (it >= RAW2) mbar_wait_long(empty, ((it / RAW2) - 1) & 1);
+                    const uint32_t sa = smem_base + s * RAW2_BYTES, sb = sa + A_BYTES;
                     const int k0 = kt * KS;
                     mbar_expect_tx(full, A_BYTES + B2_BYTES);
-                    tma_load_2d(sa_hi, &tmapA, full, k0, m0);
-                    tma_load_2d(sb_hi, &tmapB, full, k0, nb0);
+                    tma_load_2d(sa, &tmapA, full, k0, m0);
+                    tma_load_2d(sb, &tmapB, full, k0, nb0);
                 }
             }
         }
@@ -616,20 +706,20 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     const uint32_t d = tmem_base + b * TN;
                     const int kt_end = min(KT, kt + CHUNK);
                     for (bool first = true; kt < kt_end; ++kt, ++it) {
-                        const int s = it % STAGES2;
-                        mbar_wait(bar_base + 8 * s, (it / STAGES2) & 1);          // this CTA's TMA tiles landed
-                        mbar_wait_cluster(bar_conv + 8 * s, (it / STAGES2) & 1);  // lo / rot tiles written in both CTAs
+                        const int s = it % RAW2, s2 = it % SEC2;
+                        mbar_wait(bar_base + 8 * s, (it / RAW2) & 1);             // this CTA's TMA tiles landed
+                        mbar_wait_cluster(bar_conv + 8 * s2, (it / SEC2) & 1);    // second tiles written in both CTAs
                                                                                   // (the peer's converters saw its TMA tiles)
                         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                        const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sa_lo = sa_hi + A_BYTES;
-                        const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B2_BYTES;
+                        const uint32_t sa_hi = smem_base + s * RAW2_BYTES, sb_hi = sa_hi + A_BYTES;
+                        const uint32_t sa_lo = sec_base + s2 * SEC2_BYTES, sb_lo = sa_lo + A_BYTES;
 #pragma unroll
                         for (int ks = 0; ks < KS / 8; ++ks) {
                             const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
                             const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
                             const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
                             const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
-                            if (p.mixed) {
+                            if (MIXED) {
                                 umma_bf16_pair(d, al, bl, first ? 0u : 1u);    // x_b * lo_b + lo_b * x_b (pair tiles, K = 16)
                             } else {
                                 umma_tf32_pair(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
@@ -638,7 +728,7 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                             umma_tf32_pair(d, ah, bh, 1u);                     // hi * hi
                             first = false;
                         }
-                        umma_commit_pair(bar_base + 8 * (STAGES2 + s));   // frees the stage in both CTAs when these MMAs retire
+                        umma_commit_pair(bar_empty + 8 * s);              // frees the stage in both CTAs when these MMAs retire
                     }
                     umma_commit_pair(bar_tfull + 8 * b);                  // this chunk's accumulator is complete (both CTAs)
                 }
@@ -646,7 +736,7 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         }
     } else if (warp >= kFirstConvWarp2) {
         // ------------------------------------------------------------------ converter warps (both CTAs)
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 104;");
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kConvRegs2));
         constexpr int CT = kConvWpg2 * 32;                       // threads that share one stage
         constexpr int NA = A_BYTES / 16 / CT, NBV = B2_BYTES / 16 / CT;
         constexpr int BATCH = NA < 8 ? NA : 8;                   // 16-byte chunks of A (and of B) in flight per thread
@@ -657,10 +747,14 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
         for (int tile = pair; tile < total_tiles; tile += npairs) {
             for (int kt = 0; kt < KT; ++kt, ++it) {
                 if ((int)(it % kConvGroups2) != grp) continue;
-                const int s = it % STAGES2;
-                mbar_wait(bar_base + 8 * s, (it / STAGES2) & 1);
-                const uint32_t sa_hi = smem_base + s * STAGE2_BYTES, sa_lo = sa_hi + A_BYTES;
-                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B2_BYTES;
+                const int s = it % RAW2, s2 = it % SEC2;
+                mbar_wait(bar_base + 8 * s, (it / RAW2) & 1);
+                // slot s2 of the second ring is free once the MMAs of stage it - SEC2 have retired, which is what the
+                // raw ring's empty barrier of that stage reports (it cannot be a whole phase further: the in-order
+                // MMA issuer has not seen stage `it` converted yet, and SEC2 < RAW2)
+                if (it >= (unsigned)SEC2) mbar_wait(bar_empty + 8 * ((it - SEC2) % RAW2), ((it - SEC2) / RAW2) & 1);
+                const uint32_t sa_hi = smem_base + s * RAW2_BYTES, sb_hi = sa_hi + A_BYTES;
+                const uint32_t sa_lo = sec_base + s2 * SEC2_BYTES, sb_lo = sa_lo + A_BYTES;
 #pragma unroll
                 for (int b0 = 0; b0 < NA; b0 += BATCH) {
                     float4 va[BATCH], vb[BATCH];
@@ -670,7 +764,7 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                     for (int i = 0; i < BATCH; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + (b0 + i) * CT) * 16);
 #pragma unroll
                     for (int i = 0; i < BATCH; ++i)
-                        sts128(sa_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<false>(va[i], p.mixed));
+                        sts128(sa_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<false>(va[i], MIXED));
                     if (CPLX && rank == 1) {
                         // this CTA supplies -iX: rotate the raw tile in place (a thread rewrites the chunk it read)
 #pragma unroll
@@ -678,24 +772,24 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                             const uint32_t off = (uint32_t)(ct + (b0 + i) * CT) * 16;
                             const float4 r = rot_mi(vb[i]);
                             sts128(sb_hi + off, r);
-                            sts128(sb_lo + off, second_tile<true>(r, p.mixed));
+                            sts128(sb_lo + off, second_tile<true>(r, MIXED));
                         }
                     } else {
 #pragma unroll
                         for (int i = 0; i < BATCH; ++i)
-                            sts128(sb_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<true>(vb[i], p.mixed));
+                            sts128(sb_lo + (uint32_t)(ct + (b0 + i) * CT) * 16, second_tile<true>(vb[i], MIXED));
                     }
                 }
                 static_assert(NA == NBV && NA % BATCH == 0, "A and B halves of a stage have the same size");
                 // generic-proxy writes -> visible to the tensor core's async-proxy reads
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(leader_conv + 8 * s);
+                if (lane == 0) mbar_arrive_cluster(leader_conv + 8 * s2);
             }
         }
     } else if (warp >= kFirstAccWarp && warp < kFirstConvWarp2) {
         // ------------------------------------------------------------------ accumulator / epilogue warps (both CTAs)
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 184;");
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kAccRegs2));
         const int quarter = warp & 3;
         const int half = (warp - kFirstAccWarp) >> 2;
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
@@ -711,14 +805,14 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
             for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
             for (int ch = 0; ch < NCH; ++ch, ++gc) {
                 const int b = gc & 1;
-                mbar_wait(bar_tfull + 8 * b, (gc >> 1) & 1);
+                mbar_wait_long(bar_tfull + 8 * b, (gc >> 1) & 1);
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll
-                for (int j = 0; j < TN / 2 / 32; ++j) {
-                    float t[32];
-                    tmem_ld32(taddr + b * TN + j * 32, t);
+                for (int j = 0; j < TN / 2 / 16; ++j) {      // 16 columns at a time: the 128 sums leave few registers
+                    float t[16];
+                    tmem_ld16(taddr + b * TN + j * 16, t);
 #pragma unroll
-                    for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
+                    for (int i = 0; i < 16; ++i) racc[j * 16 + i] += t[i];
                 }
                 asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
                 __syncwarp();
@@ -734,8 +828,8 @@ step_tf32_pair_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_co
                 if (col < p.n && row_ok) {
                     const float c = p.c_col ? (float)p.c_col[col] : p.c;
                     const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
-                    float y = alpha * (racc[i] - c * p.X[off]);
-                    if (p.use_beta) y = fmaf(beta, p.Y[off], y);
+                    float y = alpha * (racc[i] - c * __ldcg(p.X + off));   // L2 only: see step_dmma.cu
+                    if (p.use_beta) y = fmaf(beta, __ldcg(p.Y + off), y);
                     p.Y[off] = y;
                 }
             }
@@ -799,8 +893,11 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     std::call_once(once, [] {
         attr_err = cudaFuncSetAttribute(step_tf32_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL);
         if (attr_err == cudaSuccess)
-            attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            SMEM2_TOTAL);
+            attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX, true>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_TOTAL);
+        if (attr_err == cudaSuccess)
+            attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX, false>,
+                                            cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_TOTAL);
     });
     if (attr_err != cudaSuccess) return attr_err;
     const int64_t n = plan->ncols - s;
@@ -833,8 +930,12 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     }
     if (pair) {   // persistent CTA pairs: one cluster of 2 per TPC
         const int grid = 2 * std::min(total_tiles, std::max(1, sm_count() / 2));
-        step_tf32_pair_kernel<CPLX><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
-            *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
+        if (plan->mixed)
+            step_tf32_pair_kernel<CPLX, true><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
+                *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
+        else
+            step_tf32_pair_kernel<CPLX, false><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
+                *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
         count_launch();
         return cudaGetLastError();
     }

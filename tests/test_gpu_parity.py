@@ -124,6 +124,22 @@ def test_tf32_path_shapes(dtype, N, ncols):
     assert_parity(got, run_oracle(w, degrees=deg.numpy()), dtype)
 
 
+@pytest.mark.parametrize("dtype,N,ncols", [(torch.complex64, 1280, 300), (torch.float32, 1024, 520)])
+def test_tf32_classic_three_product_split(dtype, N, ncols, monkeypatch):
+    """CHASE_TF32_MIXED=0 selects the classic 3xTF32 split (hi*lo + lo*hi + hi*hi as three TF32 MMAs); the default
+    evaluates the two cross terms as one BF16 MMA.  Both must meet the single-precision bound; the switch is read
+    when a call creates its plan."""
+    w = W.make_config(5, N=N, ncols=ncols, dtype=dtype)
+    ref = run_oracle(w)
+    errs = {}
+    for mode in ("0", "1"):
+        monkeypatch.setenv("CHASE_TF32_MIXED", mode)
+        got = run_gpu(w)
+        assert_parity(got, ref, dtype)
+        errs[mode] = rel_fro(got, ref)
+    assert errs["0"] != errs["1"], "the two split schemes round differently; equal errors mean the switch is dead"
+
+
 def test_tf32_launch_count_and_workspace():
     """One step kernel per degree on the tensor path too; scratch = one vector block + 256 bytes."""
     N, n = 512, 64
