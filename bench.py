@@ -50,10 +50,12 @@ TF32_OVER_BF16_NOMINAL = 1.1 / 2.25      # B200_PROFILING.md nominal dense peaks
 # dram__bytes_read.sum + dram__bytes_write.sum of one full-width step launch (ncu --set full captures).
 # NOT measured in this run: typed in from the committed capture named in each note.
 NCU_TRAFFIC = {
-    4: (199.664869e9 + 1.309856e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9); from "
-                                   "profiles/ncu_r1d_step_dmma.md, not measured in this run"),
-    5: (129.506315e9 + 1.473567e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
-                                   "from profiles/ncu_r1c_step_tf32_c64.md, not measured in this run"),
+    4: (157.315675e9 + 1.352249e9, "bytes of one full-width launch (2000 columns; algorithmic 30.7e9; 145-157e9 over three "
+                                   "captures); from profiles/ncu_r2_step_dmma.md, not measured in this run"),
+    5: (134.158879e9 + 1.454750e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
+                                   "from profiles/ncu_r2_step_tf32.md, not measured in this run"),
+    2: (328.881152e6 + 18.007808e6, "bytes of one full-width launch (256 columns; algorithmic 268e6 + vectors); "
+                                    "from profiles/ncu_r2_step_dmma.md, not measured in this run"),
 }
 
 

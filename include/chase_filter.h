@@ -51,9 +51,9 @@ extern "C" {
 #define CHASE_MAX_DEGREE 4096 /* largest accepted degrees[j]; the paper's degrees are <= 36 (Table 1) */
 
 typedef enum {
-    CHASE_F32 = 0,  /* float,                 tcgen05 3xTF32 tensor path when N % 4 == 0, else FP32 FMA */
+    CHASE_F32 = 0,  /* float,                 tcgen05 split-precision tensor path when N % 4 == 0, else FP32 FMA */
     CHASE_F64 = 1,  /* double,                FP64 (DMMA tensor path when N is even) */
-    CHASE_C64 = 2,  /* interleaved float2,    tcgen05 3xTF32 tensor path when N % 2 == 0, else FP32 FMA */
+    CHASE_C64 = 2,  /* interleaved float2,    tcgen05 split-precision tensor path when N % 2 == 0, else FP32 FMA */
     CHASE_C128 = 3  /* interleaved double2,   FP64 (DMMA tensor path for every N >= 16) */
 } chase_dtype_t;
 
@@ -270,10 +270,12 @@ int chase_ipc_open(const void *handle64, void **base_out);
 int chase_ipc_close(void *base);
 
 /* Which kernel family chase_filter_ws would use: 1 = TMA + FP64 DMMA tensor kernel (c128 with
- * any N >= 16, f64 with even N), 2 = tcgen05 3xTF32 kernel (c64 with N % 2 == 0, f32 with
- * N % 4 == 0; FP32 operands split on chip into two TF32 parts, FP32 accumulation), 0 = generic FMA
- * kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1 turns 2
- * into 0.  Negative = invalid arguments. */
+ * any N >= 16, f64 with even N), 2 = tcgen05 split-precision kernel (c64 with N % 2 == 0, f32 with
+ * N % 4 == 0; every FP32 operand x is split on chip as hi + lo, hi*hi is a TF32 MMA and the two
+ * cross terms are ONE BF16 MMA, FP32 accumulation; error vs an FP64 evaluation ~2e-5 at degree 16),
+ * 0 = generic FMA kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1
+ * turns 2 into 0, CHASE_TF32_MIXED=0 evaluates the cross terms as two TF32 MMAs (classic 3xTF32),
+ * CHASE_TF32_PAIR=0 selects the single-CTA variant of kernel 2.  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
 
 /* Work decomposition the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active`
