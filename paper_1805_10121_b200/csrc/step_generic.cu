@@ -52,10 +52,10 @@ step_generic_kernel(const R *__restrict__ H, const R *__restrict__ X, R *Y,
             const int64_t gk = k0 + k, gj = n0 + j;
             const bool ok = gk < N && gj < n;
             if (CPLX) {
-                Bs[0][k][j] = ok ? X[2 * (gk + gj * N)] : R(0);
-                Bs[NC - 1][k][j] = ok ? X[2 * (gk + gj * N) + 1] : R(0);
+                Bs[0][k][j] = ok ? __ldcg(X + 2 * (gk + gj * N)) : R(0);
+                Bs[NC - 1][k][j] = ok ? __ldcg(X + 2 * (gk + gj * N) + 1) : R(0);
             } else {
-                Bs[0][k][j] = ok ? X[gk + gj * N] : R(0);
+                Bs[0][k][j] = ok ? __ldcg(X + gk + gj * N) : R(0);
             }
         }
         __syncthreads();
@@ -102,8 +102,8 @@ step_generic_kernel(const R *__restrict__ H, const R *__restrict__ X, R *Y,
             const int64_t off = (gm + gj * N) * NC;
 #pragma unroll
             for (int q = 0; q < NC; ++q) {
-                R v = alpha * (acc[q][i][j] - c * X[off + q]);
-                if (use_beta) v = fma(beta, Y[off + q], v);
+                R v = alpha * (acc[q][i][j] - c * __ldcg(X + off + q));
+                if (use_beta) v = fma(beta, __ldcg(Y + off + q), v);
                 Y[off + q] = v;
             }
         }

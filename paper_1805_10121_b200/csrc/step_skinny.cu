@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(kThreads) step_skinny_kernel(const T *__restri
                 if (m < N && j < n) {
                     const int64_t off = (int64_t)j * N + m;
                     const R cc = c_col ? (R)c_col[j] : c;
-                    Y[off] = epilogue<T, R>(acc[cidx][j], X[off], use_beta ? Y[off] : zero(T()), alpha, beta, cc, use_beta);
+                    Y[off] = epilogue<T, R>(acc[cidx][j], __ldcg(X + off), use_beta ? __ldcg(Y + off) : zero(T()), alpha, beta, cc, use_beta);
                 }
             }
         }

@@ -231,7 +231,7 @@ step_stream_kernel(const __grid_constant__ CUtensorMap tmapH, const __grid_const
                 const T total = add(r[warp * 32 + lane], r[(warp + 4) * 32 + lane]);
                 const int64_t off = (int64_t)j * N + m;
                 const R cc = c_col ? (R)c_col[j] : c;
-                Y[off] = epi(total, X[off], use_beta ? Y[off] : zero(T()), alpha, beta, cc, use_beta);
+                Y[off] = epi(total, __ldcg(X + off), use_beta ? __ldcg(Y + off) : zero(T()), alpha, beta, cc, use_beta);   // L2 only: step_dmma.cu
             }
         }
         // `red` alternates between two halves, and a warp can only get one block ahead of the slowest
