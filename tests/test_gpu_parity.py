@@ -293,3 +293,35 @@ def test_default_mode_whole_tile_rounds_then_stream_k():
     got = V.cpu().numpy()
     assert float(np.linalg.norm(got - ref) / np.linalg.norm(ref)) <= 1e-12
     assert torch.equal(H.cpu(), w.H)
+
+
+@pytest.mark.parametrize("dtype,N,ncols", [(torch.complex128, 512, 60), (torch.float64, 1040, 150),
+                                           (torch.complex64, 768, 160)])
+def test_filter_call_replays_from_a_cuda_graph(dtype, N, ncols):
+    """chase_filter_ws only enqueues work on the caller's stream (kernels -- with their programmatic-dependent-launch
+    edges --, a 1 KB memset, device copies of odd-degree columns), so a call can be captured ONCE and replayed: the
+    filter "is called hundreds of times" with the same shapes.  Two replays on restored inputs must
+    both equal the oracle, and each other bit for bit."""
+    w = W.make_config(2, N=N, ncols=ncols, dtype=dtype)
+    rng = np.random.default_rng(11)
+    deg = torch.tensor(np.sort(rng.integers(1, 12, size=ncols)).astype(np.int32))      # even and odd degrees, drops
+    ref = run_oracle(w, degrees=deg.numpy())
+    H, V0 = to_device(w.H), to_device(w.V0)
+    V = W.empty_colmajor(N, ncols, dtype, _dev())
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(N, ncols, dtype), dtype=torch.uint8, device=_dev())
+    V.copy_(V0)
+    pkg.chase_filter_ws(H, V, deg, w.a, w.b, w.lambda1, ws)          # warm-up outside the capture (one-time attribute calls)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    V.copy_(V0)
+    with torch.cuda.graph(graph):
+        pkg.chase_filter_ws(H, V, deg, w.a, w.b, w.lambda1, ws)
+    outs = []
+    for _ in range(2):
+        V.copy_(V0)
+        ws.fill_(0xFF)                                                # the replay must re-initialise what it relies on
+        graph.replay()
+        torch.cuda.synchronize()
+        outs.append(V.clone())
+    assert_parity(outs[0].cpu().numpy(), ref, dtype)
+    assert torch.equal(outs[0], outs[1])
