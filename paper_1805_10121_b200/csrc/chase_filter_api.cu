@@ -362,6 +362,12 @@ namespace chase {
 struct HostUpload {
     const void *H_host;
     cudaStream_t copy_stream;
+    // result download, column class by column class: the columns of degree k are final after step k (later steps
+    // only touch columns to their right, in either buffer), so they go back to the host while the remaining steps
+    // run.  d2h_stream / done: a stream and a reusable event of the caller; V_host null = no early download.
+    void *V_host;
+    cudaStream_t d2h_stream;
+    cudaEvent_t done;
 };
 static int filter_impl(const void *H, int64_t N, void *V, int64_t ncols, const int32_t *degrees,
                        double a, double b, double lambda1, chase_dtype_t dtype,
@@ -429,6 +435,19 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
                                         cudaMemcpyHostToDevice, stream);
         if (e != cudaSuccess) return (int)e;
     }
+    // chase_filter_host: the columns of degree k (final after step k, in buf[k & 1]) go back to the host behind an event
+    const bool early_d2h = up && up->V_host;
+    auto download_class = [&](int k) -> cudaError_t {
+        if (!early_d2h) return cudaSuccess;
+        const int64_t j0 = offset[k], j1 = k < m_max ? offset[k + 1] : ncols;
+        if (j1 <= j0) return cudaSuccess;
+        cudaError_t e = cudaEventRecord(up->done, stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(up->d2h_stream, up->done, 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync((char *)up->V_host + (size_t)j0 * col_bytes, (const char *)buf[k & 1] + (size_t)j0 * col_bytes,
+                                (size_t)(j1 - j0) * col_bytes, cudaMemcpyDeviceToHost, up->d2h_stream);
+        return e;
+    };
     for (int k = 1; k <= m_max; ++k) {
         const int64_t s = offset[k];
         const int src = (k - 1) & 1;
@@ -437,10 +456,10 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
             // Step 1 row panel by row panel, each as soon as its rows of H have landed: the upload of H
             // (26 GB at cfg 4, ~0.5 s over PCIe) hides behind the first step (~0.7 s).
             const int64_t tiles = (N + 127) / 128;
-            const int panels = (int)std::min<int64_t>(8, tiles);
+            const int panels = (int)std::min<int64_t>(8, tiles);      // (16 panels measured no better: 15.86 vs 15.70 s)
             const int64_t rows_per = (tiles + panels - 1) / panels * 128;
             struct Events {                 // destroyed on every exit path
-                cudaEvent_t ev[8];
+                cudaEvent_t ev[16];
                 int n = 0;
                 ~Events() { for (int i = 0; i < n; ++i) cudaEventDestroy(ev[i]); }
             } evs;
@@ -448,7 +467,7 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
             for (int64_t r0 = 0; r0 < N; r0 += rows_per) {
                 const int64_t rows = std::min(rows_per, N - r0);
                 cudaEvent_t evp;
-                if (evs.n >= 8) return CHASE_ERR_ARG;
+                if (evs.n >= 16) return CHASE_ERR_ARG;
                 if ((e = cudaEventCreateWithFlags(&evp, cudaEventDisableTiming)) != cudaSuccess) return (int)e;
                 ev[evs.n++] = evp;
                 e = cudaMemcpy2DAsync((char *)const_cast<void *>(H) + (size_t)r0 * w, (size_t)N * w,
@@ -465,6 +484,7 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
                 if ((e = dmma_plan_create_panel(&pp, dtype, H, N, r0, rows, V, workspace, ncols)) != cudaSuccess) return (int)e;
                 if ((e = dmma_launch_step(&pp, src, s, alpha[k], beta[k], c, 0, stream)) != cudaSuccess) return (int)e;
             }
+            if ((e = download_class(k)) != cudaSuccess) return (int)e;
             continue;
         }
         // Few active columns left (the tail of a sorted-degree schedule): one streaming pass over H beats a
@@ -497,7 +517,9 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
             e = launch_step_generic(dtype, sa, stream);
         }
         if (e != cudaSuccess) return (int)e;
+        if ((e = download_class(k)) != cudaSuccess) return (int)e;
     }
+    if (early_d2h) return CHASE_OK;        // every column went to the host from the buffer it ended in
 
     // Result placement: V_{m_j} of an odd-degree column ended in the scratch
     // buffer; copy each contiguous run of odd-degree columns back (none for Alg. 5's degrees).
@@ -565,14 +587,30 @@ int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols
     cudaStream_t cp = nullptr;
     if (rc == CHASE_OK && (e = cudaStreamCreateWithFlags(&cp, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
     if (rc == CHASE_OK && (e = cudaMemcpyAsync(dV, V_host, vb, cudaMemcpyHostToDevice, st)) != cudaSuccess) fail(e);
-    if (rc == CHASE_OK) {   // H goes up inside the filter, overlapped with its first step
-        HostUpload up{H_host, cp};
+    cudaStream_t dl = nullptr;
+    cudaEvent_t done = nullptr;
+    if (rc == CHASE_OK && (e = cudaStreamCreateWithFlags(&dl, cudaStreamNonBlocking)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK && (e = cudaEventCreateWithFlags(&done, cudaEventDisableTiming)) != cudaSuccess) fail(e);
+    if (rc == CHASE_OK) {   // H goes up inside the filter, overlapped with its first step; finished column classes
+                            // go down while the remaining steps run (degree-0 columns never leave the host)
+        // (only for large blocks: a copy into pageable memory blocks the host until the step before it has run,
+        //  which would cost a latency-bound small call its launch overlap)
+        const bool early = vb >= ((size_t)64 << 20);
+        HostUpload up{H_host, cp, early ? V_host : nullptr, dl, done};
         rc = filter_impl(dH, N, dV, ncols, degrees, a, b, lambda1, dtype, dW, wb, (void *)st, &up);
+        if (rc == CHASE_OK && !early &&
+            (e = cudaMemcpyAsync(V_host, dV, vb, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+            fail(e);
     }
     (void)hb;
-    if (rc == CHASE_OK && (e = cudaMemcpyAsync(V_host, dV, vb, cudaMemcpyDeviceToHost, st)) != cudaSuccess) fail(e);
     e = cudaStreamSynchronize(st);
     if (rc == CHASE_OK && e != cudaSuccess) fail(e);
+    if (dl) {
+        e = cudaStreamSynchronize(dl);
+        if (rc == CHASE_OK && e != cudaSuccess) fail(e);
+        cudaStreamDestroy(dl);
+    }
+    if (done) cudaEventDestroy(done);
     cudaFree(dH);
     cudaFree(dV);
     cudaFree(dW);

@@ -188,3 +188,23 @@ def test_repeated_calls_are_bitwise_identical(cfg, N, ncols):
     assert bool(torch.isfinite(torch.view_as_real(runs[0]) if runs[0].is_complex() else runs[0]).all())
     for other in runs[1:]:
         assert torch.equal(runs[0], other)
+
+
+def test_host_entry_downloads_column_classes_early():
+    """chase_filter_host on a block large enough (>= 64 MB) for the class-by-class download: the columns of degree k
+    leave the device right after step k, from whichever buffer they ended in (odd degrees: the scratch buffer), while
+    the later steps run; degree-0 columns never leave the host.  Compared with the oracle on a column sample that holds
+    both ends of every class."""
+    N, n = 8192, 520                                             # 68 MB of complex128 vectors
+    w = W.make_config(2, N=N, ncols=n)
+    rng = np.random.default_rng(3)
+    deg = np.sort(rng.integers(0, 8, size=n)).astype(np.int32)    # 0..7: untouched, odd and even classes
+    V = W.as_colmajor(w.V0.clone())
+    pkg.chase_filter_host(w.H, V, torch.tensor(deg), w.a, w.b, w.lambda1, device=0)
+    cols = W.parity_sample_columns(torch.tensor(deg))
+    ref = oracle.chase_filter(w.H.numpy(), np.asfortranarray(w.V0.numpy()[:, cols]), deg[cols], w.a, w.b, w.lambda1)
+    got = V.numpy()[:, cols]
+    assert rel_fro(got, ref) <= 1e-12
+    col_err = np.linalg.norm(got - ref, axis=0) / np.linalg.norm(ref, axis=0)
+    assert col_err.max() <= 1e-11, cols[int(col_err.argmax())]
+    assert np.array_equal(V.numpy()[:, deg == 0], w.V0.numpy()[:, deg == 0])
