@@ -400,6 +400,10 @@ def roofline_of(pkg, w, achieved_tflops: float, clocks, device, launches_per_ste
         "traffic": traffic, "traffic_note": traffic_note, "peak_source": peak_source,
         "frac_of_nvidia_quoted_40tf": achieved_tflops / 40.0 if is_f64 else None,
         "frac_of_3xtf32_peak": frac_3x,
+        # single-precision configs also against the FP32 FMA pipe (148 SMs x 256 flop/clk at max clock,
+        # 74.5 TFLOP/s nominal) -- what a kernel WITHOUT tensor cores could reach at best
+        "frac_of_fp32_fma_peak": (achieved_tflops / (sms * 2 * FP64_FLOP_PER_CLK_SM * sm_max_mhz * 1e-6)
+                                  if not is_f64 else None),
         "algorithmic_flops_per_step": w.flops(), "launches_per_step": launches_per_step,
     }
 
@@ -493,6 +497,7 @@ def run_ours(args):
     flops_step = w.flops()
     r = time_filter(pkg, w, args.steps, args.warmup, device, world, rank, local)
     V, launches, clocks, t_wall = r["V"], r["launches"], r["clocks"], r["t_wall"]
+    r_ms = list(r["ms"])
     dev_s = max_over_ranks(r["dev_s"], world)
     total_flops = sum_over_ranks(flops_step * args.steps, world)
     value = total_flops / dev_s * 1e-9
@@ -521,7 +526,8 @@ def run_ours(args):
         sample = (f"{len(cols)} of {n} columns (evenly spaced), full {N}x{N} H, degree truncated to "
                   f"{args.sample_degree}")
         cpu_baseline = {"value": fl / dt * 1e-9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                        "sample": sample, "seconds": dt}
+                        "sample": sample, "seconds": dt,
+                        "extrapolated_seconds_for_the_whole_workload": dt * flops_step / fl}
         try:
             blas_ctx = cpu_blas_context(w)
         except Exception as exc:
@@ -587,7 +593,8 @@ def run_ours(args):
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": dev_s / args.steps * 1e3, "higher_is_better": True,
+            "warmup": args.warmup, "ms_per_step": dev_s / args.steps * 1e3, "ms_min": min(r_ms),
+            "ms_median": statistics.median(r_ms), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": DTYPE_LABEL[dtype],
             "data": "synthetic", "config": cfg_line, "clocks": clocks,
             "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
