@@ -99,8 +99,11 @@ int chase_filter(const void *H, int64_t N, void *V, int64_t ncols, const int32_t
  * pointers (pinned or pageable).  Allocates device buffers, copies V and H to the device,
  * runs the filter, copies V back, frees, and SYNCHRONISES before returning.  On the FP64 tensor
  * path H is uploaded in 8 row panels on a second stream and the first degree step runs panel by
- * panel as the rows arrive, so the upload of H hides behind that step.
- * `device` is the CUDA device ordinal. */
+ * panel as the rows arrive, so the upload of H hides behind that step.  For vector blocks of
+ * 64 MB and more the result comes back column class by column class: the columns of degree k are
+ * final after step k and are copied to V_host on a third stream while the later steps run (V_host
+ * must not be read or written by the caller during the call; columns of degree 0 are not touched).
+ * On an error return the contents of V_host are unspecified.  `device` is the CUDA device ordinal. */
 int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols,
                       const int32_t *degrees, double a, double b, double lambda1,
                       chase_dtype_t dtype, int device);
