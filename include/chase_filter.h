@@ -65,8 +65,10 @@ enum {
     CHASE_ERR_DTYPE = -4,     /* unknown chase_dtype_t */
     CHASE_ERR_WORKSPACE = -5, /* workspace null or smaller than chase_filter_workspace_bytes */
     CHASE_ERR_ALIGN = -6,     /* H, V or workspace not aligned to 16 bytes */
-    CHASE_ERR_TIMEOUT = -7    /* row-sharded path: a peer rank did not reach an inter-GPU barrier in time
+    CHASE_ERR_TIMEOUT = -7,   /* row-sharded path: a peer rank did not reach an inter-GPU barrier in time
                                  (chase_rows_status), or the caller's host barrier reported a failure */
+    CHASE_ERR_STATIC_LIMIT = -8 /* chase_residuals_static: the problem needs more scratch than the library's
+                                 built-in CHASE_STATIC_SCRATCH_BYTES */
 };
 
 /* Bytes of device scratch chase_filter_ws needs: one N x ncols buffer of `dtype` (the W of
@@ -155,6 +157,39 @@ size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t d
 int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, const double *ritzv,
                     double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
                     void *stream);
+
+/* chase_residuals for callers that may not allocate device memory.
+ *
+ * Some users of this library live inside a memory budget they do not control: a plug-in of an application
+ * whose own pool has already reserved the whole GPU, a process whose HBM share was fixed when the job
+ * started, a latency-critical loop that must stay out of the driver's allocator (cudaMalloc and cudaFree
+ * stall the whole device while they run).  Such a caller can neither pass a workspace to chase_residuals
+ * nor let the library fetch one.  For them the library carries CHASE_STATIC_SCRATCH_BYTES of device memory
+ * of its own, a static array inside the library image, and this one entry point uses it as the workspace:
+ * same arguments as chase_residuals minus the workspace, same kernels, same results.  It calls no
+ * cudaMalloc / cudaMallocAsync / cudaFree and no library routine that allocates.
+ *
+ *   H, V       DEVICE, read-only, as in chase_residuals, on the CURRENT device
+ *   ritzv      HOST double[ncols]; resid  DEVICE double[ncols] (the only output)
+ *   Limit: chase_residuals_workspace_bytes(N, ncols, dtype) <= CHASE_STATIC_SCRATCH_BYTES (48 MiB), i.e. a vector
+ *          block N * ncols * sizeof(element) of just under 28 MiB on the FP64 tensor path (whose stream-K scratch
+ *          takes 20 MiB of the array) and just under 48 MiB on the other paths; N = 3893, ncols = 282 complex128
+ *          (the paper's NaCl problem) needs 36.8 MiB and fits.  Anything larger returns
+ *          CHASE_ERR_STATIC_LIMIT before any CUDA call.
+ *   Cost: a GPU holds the 48 MiB from the moment the CUDA module with the array is loaded on it (at the latest
+ *          the first call of this entry point there; with eager module loading, as soon as the process has a
+ *          context on it) until the process exits, whether or not the entry point is ever used again.
+ *   First call on a device: looks up the array's device address (cudaGetSymbolAddress, which also makes the
+ *          runtime load the module there); make that first call during set-up, before any stream capture
+ *          and before the phase in which nothing may allocate.  Later calls only enqueue work.
+ *   Sharing: all calls on one GPU use the SAME array.  It keeps the previous call's contents; the part that
+ *          must start at zero (kernel flags / counters) is cleared in stream order by every call.  Two calls
+ *          whose work can overlap on the GPU (different streams, or different host threads) RACE on it --
+ *          keep them on one stream or order them with events.  chase_residuals has no such restriction.
+ * Asynchronous on `stream` like chase_residuals; same return codes plus CHASE_ERR_STATIC_LIMIT. */
+#define CHASE_STATIC_SCRATCH_BYTES (48u << 20)
+int chase_residuals_static(const void *H, int64_t N, const void *V, int64_t ncols, const double *ritzv,
+                           double *resid, chase_dtype_t dtype, void *stream);
 
 /* Spectral estimates (Alg. 6 "Lanczos procedure for parameters estimates",
  * PAPER.md:421-475; Eq. (9)-(10)).

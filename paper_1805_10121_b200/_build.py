@@ -12,7 +12,8 @@ CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libchase_filter.so")
 OBJDIR = os.path.join(PKG, "build")
-SOURCES = ["chase_filter_api.cu", "step_generic.cu", "step_dmma.cu", "step_tf32.cu", "step_skinny.cu", "step_stream.cu", "lanczos.cu", "rows.cu", "peak_probe.cu"]
+SOURCES = ["chase_filter_api.cu", "step_generic.cu", "step_dmma.cu", "step_tf32.cu", "step_skinny.cu", "step_stream.cu", "lanczos.cu", "rows.cu", "peak_probe.cu",
+           "residuals_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

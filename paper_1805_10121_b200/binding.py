@@ -25,8 +25,9 @@ EXPORTS = [
     "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates", "chase_lanczos_ritz_vectors",
     "chase_hemm_rows", "chase_rows_barrier", "chase_rows_signal", "chase_rows_wait", "chase_rows_status",
     "chase_filter_rows_ws", "chase_filter_rows_hostsync_ws", "chase_ipc_export", "chase_ipc_open",
-    "chase_ipc_close",
+    "chase_ipc_close", "chase_residuals_static",
 ]
+CHASE_STATIC_SCRATCH_BYTES = 48 << 20      # include/chase_filter.h
 HOST_BARRIER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
 
 _lib = None
@@ -81,6 +82,8 @@ def load() -> ctypes.CDLL:
     lib.chase_residuals_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
     lib.chase_residuals.restype = ctypes.c_int
     lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
+    lib.chase_residuals_static.restype = ctypes.c_int
+    lib.chase_residuals_static.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp]
     lib.chase_filter_step_plan.restype = ctypes.c_int
     lib.chase_filter_step_plan.argtypes = [i64, i64, ctypes.c_int, i32, vp, vp]
     lib.chase_lanczos_workspace_bytes.restype = sz
@@ -326,6 +329,33 @@ def chase_residuals(H: torch.Tensor, V: torch.Tensor, ritzv, workspace: Optional
         _check(load().chase_residuals(H.data_ptr(), N, V.data_ptr(), ncols, rv.ctypes.data, resid.data_ptr(),
                                       _DTYPE_CODE[H.dtype], workspace.data_ptr(),
                                       workspace.numel() * workspace.element_size(), _stream_ptr(stream)))
+    return resid
+
+
+def chase_residuals_static(H: torch.Tensor, V: torch.Tensor, ritzv, resid: torch.Tensor,
+                           stream: Optional[torch.cuda.Stream] = None) -> torch.Tensor:
+    """chase_residuals for callers that may not allocate device memory (a plug-in inside an application
+    whose pool owns the whole GPU, a process with a fixed HBM share, a loop that must stay out of the
+    driver's allocator): the scratch is a 48 MiB static array inside libchase_filter.so, so this wrapper
+    creates no tensor either -- the caller brings `resid` (device float64 [ncols]), which is also returned.
+    Problems whose chase_residuals_workspace_bytes exceeds CHASE_STATIC_SCRATCH_BYTES raise ChaseFilterError
+    (code -8).  All calls on one GPU share the array: keep them on one stream.  The first call on a device
+    resolves the array's address; make it before any stream capture."""
+    if not (H.is_cuda and V.is_cuda and resid.is_cuda):
+        raise ValueError("H, V and resid must be CUDA tensors (there is no CPU path)")
+    if H.dtype != V.dtype or H.dtype not in _DTYPE_CODE:
+        raise ValueError("H and V must share a dtype in {f32, f64, c64, c128}")
+    _check_colmajor(H, "H")
+    _check_colmajor(V, "V")
+    N, ncols = V.shape
+    rv = np.ascontiguousarray(np.asarray(ritzv, dtype=np.float64))
+    if rv.shape != (ncols,):
+        raise ValueError("ritzv must have one entry per column")
+    if resid.dtype != torch.float64 or resid.shape != (ncols,) or not resid.is_contiguous():
+        raise ValueError("resid must be a contiguous float64 tensor with one entry per column")
+    with torch.cuda.device(H.device):
+        _check(load().chase_residuals_static(H.data_ptr(), N, V.data_ptr(), ncols, rv.ctypes.data, resid.data_ptr(),
+                                             _DTYPE_CODE[H.dtype], _stream_ptr(stream)))
     return resid
 
 

@@ -40,6 +40,8 @@ const char *chase_filter_strerror(int code) {
         case CHASE_ERR_WORKSPACE: return "workspace missing or too small";
         case CHASE_ERR_ALIGN: return "H, V and workspace must be 16-byte aligned";
         case CHASE_ERR_TIMEOUT: return "a peer rank did not reach an inter-GPU barrier in time";
+        case CHASE_ERR_STATIC_LIMIT:
+            return "problem too large for the library's static scratch (CHASE_STATIC_SCRATCH_BYTES); use chase_residuals";
         default:
             if (code > 0) return cudaGetErrorString((cudaError_t)code);
             return "unknown error";

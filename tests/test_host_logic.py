@@ -27,7 +27,7 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_strerror_covers_codes():
-    for code in range(0, -7, -1):
+    for code in range(0, -9, -1):
         assert pkg.chase_filter_strerror(code) != "unknown error"
     assert pkg.chase_filter_strerror(-99) == "unknown error"
 
