@@ -110,6 +110,24 @@ int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols
                       const int32_t *degrees, double a, double b, double lambda1,
                       chase_dtype_t dtype, int device);
 
+/* chase_filter_host for a SEQUENCE of calls on one matrix.  The filter "is called hundreds of times" in a solve
+ * and ChASE works on sequences of problems; chase_filter_host allocates, uploads and frees H
+ * (N^2 elements: 25.6 GB at N = 40 000 complex128) on every call.  With a handle H goes up once:
+ *   chase_filter_host_open   cudaSetDevice(device), allocates H, an N x max_ncols vector block and the workspace
+ *                            of the widest call, uploads H_host (HOST, pinned or pageable; may be released after
+ *                            the call) and SYNCHRONISES.  *handle_out (HOST) receives the handle.
+ *   chase_filter_host_run    V_host (HOST, N x ncols, ncols <= max_ncols; in: V_0, out: result) goes up, the
+ *                            filter of chase_filter_ws runs on the resident H, the result comes back; SYNCHRONISES.
+ *                            Columns of degree 0 are not transferred.  Same validation and return codes as
+ *                            chase_filter_host.  Calls on one handle must not overlap (one stream, one buffer set).
+ *   chase_filter_host_close  waits for the handle's stream and frees everything.
+ * A handle may be used from any host thread, one at a time. */
+int chase_filter_host_open(const void *H_host, int64_t N, int64_t max_ncols, chase_dtype_t dtype, int device,
+                           void **handle_out);
+int chase_filter_host_run(void *handle, void *V_host, int64_t ncols, const int32_t *degrees, double a, double b,
+                          double lambda1);
+int chase_filter_host_close(void *handle);
+
 /* Host-side pieces of Alg. 4, exposed for tests and callers that want to inspect the plan.
  * chase_filter_scalars: alpha[k], beta[k] (k = 1..m_max; entry 0 unused; arrays of m_max+1
  *   doubles, HOST) such that V_k = alpha[k] (H - cI) V_{k-1} + beta[k] V_{k-2}; *c = center.
@@ -154,6 +172,12 @@ int chase_degrees(int64_t ncols, const double *resid, const double *ritzv, doubl
 int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
                double alpha, double beta, double shift, chase_dtype_t dtype, void *stream);
 size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype);
+/* chase_hemm, chase_hemm_rows and the chase_filter_rows_* calls bring no workspace, so on the FP64 tensor path
+ * their stream-K scratch (about 20 MB per launch in flight) comes from a process-wide cache of cudaMalloc'ed
+ * buffers that is kept for reuse.  chase_scratch_cache_release gives those buffers back: it waits for the launch
+ * each one last served, frees them, and the next such launch allocates afresh.  Returns 0, a cudaError_t, or
+ * cudaErrorNotReady (600) when another host thread is inside such a launch at this moment (nothing freed). */
+int chase_scratch_cache_release(void);
 int chase_residuals(const void *H, int64_t N, const void *V, int64_t ncols, const double *ritzv,
                     double *resid, chase_dtype_t dtype, void *workspace, size_t workspace_bytes,
                     void *stream);
@@ -220,11 +244,13 @@ int chase_residuals_static(const void *H, int64_t N, const void *V, int64_t ncol
  *   n_vec runs, i.e. run = 1 when run 0 is the b_sup run), with T_k = Z^H diag(lam~) Z, writes the Ritz
  *   vector  x_i = U^[run] z_i  of every Ritz value lam~_i < mu_ne, in ascending order of lam~_i and at
  *   most max_vecs of them, into column dst_cols[i] of Vhat (DEVICE, N x ncols_vhat column-major) -- the
- *   caller picks the columns, which is the interspersing.  The sign of x_i is fixed by Z_{1,i} >= 0.
+ *   caller picks the columns, which is the interspersing; the max_vecs entries of dst_cols must be distinct
+ *   (CHASE_ERR_ARG otherwise).  The sign of x_i is fixed by Z_{1,i} >= 0.
  *   `workspace` is the one a chase_lanczos call with the same (N, nruns, k, dtype) left behind (the
  *   Lanczos vectors are still in it), alpha / beta that call's outputs (HOST [nruns * k]).
  *   *count (HOST) receives the number of vectors written, ritz_values (HOST [max_vecs], may be NULL)
- *   their Ritz values.  One N x k by k x count product in a small kernel; SYNCHRONISES `stream`. */
+ *   their Ritz values.  One N x k by k x count product in a small kernel; SYNCHRONISES `stream` after that
+ *   kernel: Vhat is complete when the call returns. */
 size_t chase_lanczos_workspace_bytes(int64_t N, int64_t nruns, int32_t k, chase_dtype_t dtype);
 int chase_lanczos_ritz_vectors(const void *workspace, size_t workspace_bytes, int64_t N, int64_t nruns, int32_t k,
                                chase_dtype_t dtype, int64_t run, const double *alpha, const double *beta,
@@ -311,35 +337,10 @@ int chase_ipc_close(void *base);
  * any N >= 16, f64 with even N), 2 = tcgen05 split-precision kernel (c64 with N % 2 == 0, f32 with
  * N % 4 == 0; every FP32 operand x is split on chip as hi + lo, hi*hi is a TF32 MMA and the two
  * cross terms are ONE BF16 MMA, FP32 accumulation; error vs an FP64 evaluation ~2e-5 at degree 16),
- * 0 = generic FMA kernel.  Environment: CHASE_FILTER_FORCE_GENERIC=1 forces 0, CHASE_FILTER_NO_TF32=1
- * turns 2 into 0, CHASE_TF32_MIXED=0 evaluates the cross terms as two TF32 MMAs (classic 3xTF32),
- * CHASE_TF32_PAIR=0 selects the single-CTA variant of kernel 2.  Negative = invalid arguments. */
+ * 0 = generic FMA kernel.  Environment (both read on every call; tests and bench.py use them to reach the FMA
+ * kernels at TMA-legal sizes and to compare the two split schemes): CHASE_FILTER_FORCE_GENERIC=1 forces 0,
+ * CHASE_TF32_MIXED=0 evaluates the cross terms as two TF32 MMAs (classic 3xTF32).  Negative = invalid arguments. */
 int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype);
-
-/* Work decomposition the FP64 tensor step kernel (kernel path 1) uses for one launch on `n_active`
- * columns of an N x N problem on a GPU with `sms` SMs (host only, no CUDA call; for tests and inspection).
- * out (HOST int32[9]) = {row tiles of 128, column tiles, column tile width, data-parallel tiles, stream-K
- * CTAs, k-slabs per tile, CTAs launched (`grid`), data-parallel rounds, first stream-K CTA}.  The column
- * tiles cover [0, n_active) exactly once.  CTA b owns the whole tiles r * grid + b < data-parallel tiles
- * (r < rounds) in grouped raster order: by default persistent CTAs (grid = sms, first stream-K CTA = 0,
- * the producers kept in lock-step by a soft barrier); with CHASE_DMMA_LOCKSTEP=0 one tile per CTA (rounds = 1,
- * the stream-K CTAs follow them: first stream-K CTA = data-parallel tiles).  The remaining tiles are shared
- * by the CTAs first .. first + stream-K CTAs - 1 in contiguous k-slab ranges: sk_begin (HOST
- * int32[stream-K CTAs + 1], at most CHASE_MAX_SK_CTAS + 1; may be NULL) receives the range boundaries, slab s
- * being k-slab (s % slabs per tile) of tile (data-parallel tiles + s / slabs per tile).
- * Returns 0, CHASE_ERR_ARG or CHASE_ERR_DTYPE (not c128 / f64). */
-#define CHASE_MAX_SK_CTAS 160
-int chase_filter_step_plan(int64_t N, int64_t n_active, chase_dtype_t dtype, int32_t sms, int32_t *out,
-                           int32_t *sk_begin);
-
-/* Number of kernels launched by this library since load (all streams); for bench.py. */
-int64_t chase_filter_launch_count(void);
-
-/* Register-only FP64 peak probes on the current device (synchronous; for the roofline
- * denominator in bench.py).  kind 0: dependent-free DFMA chains, kind 1: mma.sync m8n8k4
- * f64 (SASS DMMA.8x8x4) chains.  Writes achieved GFLOP/s over `iters` inner iterations on
- * all SMs.  Returns 0 or a cudaError_t. */
-int chase_fp64_peak_probe(int kind, int iters, double *gflops);
 
 const char *chase_filter_strerror(int code);
 

@@ -11,5 +11,5 @@ from .binding import (  # noqa: F401
     chase_residuals_workspace_bytes, chase_filter_kernel_path, chase_filter_launch_count,
     chase_filter_scalars, chase_filter_schedule, chase_filter_step_plan, chase_filter_strerror,
     chase_filter_workspace_bytes, chase_filter_ws, chase_fp64_peak_probe, lib_path, load,
-    chase_residuals_static, CHASE_STATIC_SCRATCH_BYTES,
+    chase_residuals_static, CHASE_STATIC_SCRATCH_BYTES, chase_scratch_cache_release, HostFilter,
 )

@@ -25,7 +25,8 @@ EXPORTS = [
     "chase_lanczos", "chase_lanczos_workspace_bytes", "chase_spectral_estimates", "chase_lanczos_ritz_vectors",
     "chase_hemm_rows", "chase_rows_barrier", "chase_rows_signal", "chase_rows_wait", "chase_rows_status",
     "chase_filter_rows_ws", "chase_filter_rows_hostsync_ws", "chase_ipc_export", "chase_ipc_open",
-    "chase_ipc_close", "chase_residuals_static",
+    "chase_ipc_close", "chase_residuals_static", "chase_scratch_cache_release",
+    "chase_filter_host_open", "chase_filter_host_run", "chase_filter_host_close",
 ]
 CHASE_STATIC_SCRATCH_BYTES = 48 << 20      # include/chase_filter.h
 HOST_BARRIER_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p)
@@ -82,6 +83,14 @@ def load() -> ctypes.CDLL:
     lib.chase_residuals_workspace_bytes.argtypes = [i64, i64, ctypes.c_int]
     lib.chase_residuals.restype = ctypes.c_int
     lib.chase_residuals.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp, sz, vp]
+    lib.chase_filter_host_open.restype = ctypes.c_int
+    lib.chase_filter_host_open.argtypes = [vp, i64, i64, ctypes.c_int, ctypes.c_int, vp]
+    lib.chase_filter_host_run.restype = ctypes.c_int
+    lib.chase_filter_host_run.argtypes = [vp, vp, i64, vp, dbl, dbl, dbl]
+    lib.chase_filter_host_close.restype = ctypes.c_int
+    lib.chase_filter_host_close.argtypes = [vp]
+    lib.chase_scratch_cache_release.restype = ctypes.c_int
+    lib.chase_scratch_cache_release.argtypes = []
     lib.chase_residuals_static.restype = ctypes.c_int
     lib.chase_residuals_static.argtypes = [vp, i64, vp, i64, vp, vp, ctypes.c_int, vp]
     lib.chase_filter_step_plan.restype = ctypes.c_int
@@ -229,6 +238,48 @@ def chase_filter_host(H: torch.Tensor, V: torch.Tensor, degrees, a: float, b: fl
     return V
 
 
+class HostFilter:
+    """chase_filter_host_open / _run / _close: host tensors in and out like chase_filter_host, but H is uploaded
+    once and stays on the device for every run() on this handle (a solve calls the filter hundreds of times)."""
+
+    def __init__(self, H: torch.Tensor, max_ncols: int, device: int = 0):
+        if H.is_cuda or H.dtype not in _DTYPE_CODE:
+            raise ValueError("HostFilter takes a host tensor H of dtype f32, f64, c64 or c128")
+        _check_colmajor(H, "H")
+        if H.dim() != 2 or H.shape[0] != H.shape[1]:
+            raise ValueError("H must be N x N")
+        self.N, self.dtype, self.max_ncols = int(H.shape[0]), H.dtype, int(max_ncols)
+        handle = ctypes.c_void_p()
+        _check(load().chase_filter_host_open(H.data_ptr(), self.N, self.max_ncols, _DTYPE_CODE[H.dtype], int(device),
+                                             ctypes.addressof(handle)))
+        self._handle = handle
+
+    def run(self, V: torch.Tensor, degrees, a: float, b: float, lambda1: float) -> torch.Tensor:
+        if self._handle is None:
+            raise ValueError("handle is closed")
+        if V.is_cuda or V.dtype != self.dtype:
+            raise ValueError("V must be a host tensor of H's dtype")
+        _check_colmajor(V, "V")
+        if V.shape[0] != self.N:
+            raise ValueError("V must have N rows")
+        ncols = int(V.shape[1])
+        deg = _degrees_array(degrees, ncols)
+        _check(load().chase_filter_host_run(self._handle, V.data_ptr(), ncols, deg.ctypes.data, float(a), float(b),
+                                            float(lambda1)))
+        return V
+
+    def close(self) -> None:
+        if self._handle is not None:
+            h, self._handle = self._handle, None
+            _check(load().chase_filter_host_close(h))
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+
 def chase_filter_scalars(a: float, b: float, lambda1: float, m_max: int):
     """(alpha[0..m_max], beta[0..m_max], c); entry 0 unused."""
     alpha = np.zeros(m_max + 1)
@@ -302,6 +353,11 @@ def chase_hemm(H: torch.Tensor, X: torch.Tensor, Y: torch.Tensor, alpha: float =
         _check(load().chase_hemm(H.data_ptr(), N, X.data_ptr(), Y.data_ptr(), ncols, float(alpha), float(beta),
                                  float(shift), _DTYPE_CODE[H.dtype], _stream_ptr(stream)))
     return Y
+
+
+def chase_scratch_cache_release() -> None:
+    """Frees the stream-K scratch buffers the library keeps for chase_hemm / the row-sharded calls."""
+    _check(load().chase_scratch_cache_release())
 
 
 def chase_residuals_workspace_bytes(N: int, ncols: int, dtype: torch.dtype) -> int:
@@ -535,8 +591,23 @@ def chase_filter_rows_ws(H_loc: torch.Tensor, row0: int, V: torch.Tensor, degree
         if host_barrier is None:
             _check(load().chase_filter_rows_ws(*args))
         else:
-            cb = HOST_BARRIER_FN(lambda _ctx: int(host_barrier() or 0))
-            _check(load().chase_filter_rows_hostsync_ws(*args, cb, None))
+            # ctypes swallows an exception raised inside a callback and hands 0 (= success) to the C side, which
+            # would then spin in the wait kernel for its whole timeout: report failure instead, keep the exception
+            # and re-raise it once the C call has returned.
+            raised = []
+
+            def _barrier(_ctx):
+                try:
+                    return int(host_barrier() or 0)
+                except BaseException as exc:           # noqa: BLE001 -- must not propagate into C
+                    raised.append(exc)
+                    return 1
+
+            cb = HOST_BARRIER_FN(_barrier)
+            rc = load().chase_filter_rows_hostsync_ws(*args, cb, None)
+            if raised:
+                raise raised[0]
+            _check(rc)
     return int(seq_c.value)
 
 

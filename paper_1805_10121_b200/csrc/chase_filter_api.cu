@@ -6,6 +6,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <exception>
+#include <new>
 #include <vector>
 
 #include "chase_internal.h"
@@ -152,11 +153,7 @@ int launch_one_step(const void *H, int64_t N, const void *X, void *Y, int64_t nc
     // A few vectors: one streaming pass over H (roofline: HBM).  Measured at c128, N = 40000 on the bulk-copy
     // streaming kernel: 7.2 TB/s (1-2 columns), 6.7 (5), 4.5 (8: FP64 FMA-bound) against 5.5 TB/s for the
     // stream-K narrow-tile tensor kernel, which therefore takes FP64 blocks of 7 and 8 columns.
-    // CHASE_SKINNY_FP64=stream / dmma overrides (experiments).
-    const char *fp64_mode = std::getenv("CHASE_SKINNY_FP64");
-    bool fp64_tensor = path == 1 && ncols > 6;
-    if (path == 1 && fp64_mode && fp64_mode[0] == 's') fp64_tensor = false;
-    if (path == 1 && fp64_mode && fp64_mode[0] == 'd') fp64_tensor = true;
+    const bool fp64_tensor = path == 1 && ncols > 6;
     if (ncols <= kSkinnyMaxCols && !fp64_tensor && !(force && force[0] == '1')) {
         StepArgs sa;
         sa.H = H; sa.X = X; sa.Y = Y; sa.N = N; sa.n = ncols;
@@ -199,6 +196,14 @@ int chase_hemm(const void *H, int64_t N, const void *X, void *Y, int64_t ncols,
     if (((uintptr_t)H | (uintptr_t)X | (uintptr_t)Y) & 15) return CHASE_ERR_ALIGN;
     return launch_one_step(H, N, X, Y, ncols, alpha, beta, shift, nullptr, beta != 0.0, dtype,
                            (cudaStream_t)stream_);
+}
+
+int chase_scratch_cache_release(void) {
+    try {
+        return (int)dmma_sk_cache_clear();
+    } catch (const std::exception &) {
+        return (int)cudaErrorUnknown;
+    }
 }
 
 size_t chase_residuals_workspace_bytes(int64_t N, int64_t ncols, chase_dtype_t dtype) {
@@ -264,6 +269,13 @@ int chase_lanczos_ritz_vectors(const void *workspace, size_t workspace_bytes, in
     if (max_vecs < 0 || ncols_vhat < 0 || ncols_vhat > kMaxDim || (max_vecs > 0 && (!Vhat || !dst_cols))) return CHASE_ERR_ARG;
     for (int64_t i = 0; i < max_vecs; ++i)
         if (dst_cols[i] < 0 || dst_cols[i] >= ncols_vhat) return CHASE_ERR_ARG;
+    try {       // two Ritz vectors aimed at one column would race in the kernel: every destination at most once
+        std::vector<int64_t> sorted_dst(dst_cols, dst_cols + max_vecs);
+        std::sort(sorted_dst.begin(), sorted_dst.end());
+        if (std::adjacent_find(sorted_dst.begin(), sorted_dst.end()) != sorted_dst.end()) return CHASE_ERR_ARG;
+    } catch (const std::exception &) {
+        return (int)cudaErrorMemoryAllocation;
+    }
     for (int32_t j = 0; j < k; ++j) {
         const double al = alpha[run * k + j], be = beta[run * k + j];
         if (!std::isfinite(al) || !std::isfinite(be) || be < 0.0) return CHASE_ERR_ARG;
@@ -333,8 +345,7 @@ int chase_filter_kernel_path(int64_t N, int64_t ncols, chase_dtype_t dtype) {
     const char *force = std::getenv("CHASE_FILTER_FORCE_GENERIC");
     if (force && force[0] == '1') return 0;
     if (dmma_supported(N, ncols, dtype)) return 1;
-    const char *no_tf32 = std::getenv("CHASE_FILTER_NO_TF32");
-    if (tf32_supported(N, ncols, dtype) && !(no_tf32 && no_tf32[0] == '1')) return 2;
+    if (tf32_supported(N, ncols, dtype)) return 2;
     return 0;
 }
 
@@ -484,7 +495,15 @@ static int chase::filter_impl(const void *H, int64_t N, void *V, int64_t ncols, 
                 DmmaPlan pp;
                 if ((e = cudaStreamWaitEvent(stream, ev[pi], 0)) != cudaSuccess) return (int)e;
                 if ((e = dmma_plan_create_panel(&pp, dtype, H, N, r0, rows, V, workspace, ncols)) != cudaSuccess) return (int)e;
-                if ((e = dmma_launch_step(&pp, src, s, alpha[k], beta[k], c, 0, stream)) != cudaSuccess) return (int)e;
+                // the panels run one after the other on `stream`: they share the workspace's stream-K scratch, with
+                // the flag epoch and the soft-barrier count carried from panel to panel and on into the later steps
+                pp.sk_scratch = plan.sk_scratch;
+                pp.sk_epoch = plan.sk_epoch;
+                pp.sync_count = plan.sync_count;
+                e = dmma_launch_step(&pp, src, s, alpha[k], beta[k], c, 0, stream);
+                plan.sk_epoch = pp.sk_epoch;
+                plan.sync_count = pp.sync_count;
+                if (e != cudaSuccess) return (int)e;
             }
             if ((e = download_class(k)) != cudaSuccess) return (int)e;
             continue;
@@ -622,6 +641,90 @@ int chase_filter_host(const void *H_host, int64_t N, void *V_host, int64_t ncols
     }
     cudaStreamDestroy(st);
     return rc;
+}
+
+
+// ---- chase_filter_host with H kept on the device across calls (chase_filter_host_open / _run / _close) ----
+namespace {
+struct HostFilter {
+    int device = 0;
+    chase_dtype_t dtype = CHASE_C128;
+    int64_t N = 0, max_ncols = 0;
+    size_t ws_bytes = 0;
+    void *dH = nullptr, *dV = nullptr, *dW = nullptr;
+    cudaStream_t st = nullptr;
+};
+void host_filter_destroy(HostFilter *h) {
+    if (!h) return;
+    if (h->st) { cudaStreamSynchronize(h->st); cudaStreamDestroy(h->st); }
+    cudaFree(h->dH);
+    cudaFree(h->dV);
+    cudaFree(h->dW);
+    delete h;
+}
+}  // namespace
+
+int chase_filter_host_open(const void *H_host, int64_t N, int64_t max_ncols, chase_dtype_t dtype, int device,
+                           void **handle_out) {
+    const size_t w = chase::elem_bytes(dtype);
+    if (w == 0) return CHASE_ERR_DTYPE;
+    if (!H_host || !handle_out || N <= 0 || max_ncols <= 0 || N > kMaxDim || max_ncols > kMaxDim) return CHASE_ERR_ARG;
+    *handle_out = nullptr;
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return (int)e;
+    HostFilter *h = new (std::nothrow) HostFilter;
+    if (!h) return (int)cudaErrorMemoryAllocation;
+    h->device = device; h->dtype = dtype; h->N = N; h->max_ncols = max_ncols;
+    // the scratch of the widest call serves every narrower one (same kernel family: it depends on N and dtype only)
+    h->ws_bytes = chase_filter_workspace_bytes(N, max_ncols, dtype);
+    const size_t hb = (size_t)N * (size_t)N * w;
+    if ((e = cudaStreamCreateWithFlags(&h->st, cudaStreamNonBlocking)) == cudaSuccess &&
+        (e = cudaMalloc(&h->dH, hb)) == cudaSuccess &&
+        (e = cudaMalloc(&h->dV, (size_t)N * (size_t)max_ncols * w)) == cudaSuccess &&
+        (e = cudaMalloc(&h->dW, h->ws_bytes)) == cudaSuccess &&
+        (e = cudaMemcpyAsync(h->dH, H_host, hb, cudaMemcpyHostToDevice, h->st)) == cudaSuccess)
+        e = cudaStreamSynchronize(h->st);
+    if (e != cudaSuccess) {
+        host_filter_destroy(h);
+        return (int)e;
+    }
+    *handle_out = h;
+    return CHASE_OK;
+}
+
+int chase_filter_host_run(void *handle, void *V_host, int64_t ncols, const int32_t *degrees, double a, double b,
+                          double lambda1) {
+    HostFilter *h = (HostFilter *)handle;
+    if (!h || ncols < 0 || ncols > h->max_ncols || (ncols > 0 && (!V_host || !degrees))) return CHASE_ERR_ARG;
+    const int m_max = chase_filter_schedule(degrees, ncols, nullptr);
+    if (m_max < 0) return m_max;
+    if (!(std::isfinite(a) && std::isfinite(b) && std::isfinite(lambda1))) return CHASE_ERR_BOUNDS;
+    if (!(lambda1 < a && a < b)) return CHASE_ERR_BOUNDS;
+    if (ncols == 0 || m_max == 0) return CHASE_OK;
+    cudaError_t e = cudaSetDevice(h->device);
+    if (e != cudaSuccess) return (int)e;
+    const size_t w = chase::elem_bytes(h->dtype);
+    int64_t j0 = 0;                                     // degree-0 columns never leave the host
+    while (j0 < ncols && degrees[j0] == 0) ++j0;
+    const size_t off = (size_t)j0 * (size_t)h->N * w, vb = (size_t)(ncols - j0) * (size_t)h->N * w;
+    if ((e = cudaMemcpyAsync((char *)h->dV + off, (const char *)V_host + off, vb, cudaMemcpyHostToDevice, h->st)) != cudaSuccess)
+        return (int)e;
+    int rc = filter_impl(h->dH, h->N, h->dV, ncols, degrees, a, b, lambda1, h->dtype, h->dW, h->ws_bytes, (void *)h->st,
+                         nullptr);
+    if (rc == CHASE_OK &&
+        (e = cudaMemcpyAsync((char *)V_host + off, (const char *)h->dV + off, vb, cudaMemcpyDeviceToHost, h->st)) != cudaSuccess)
+        rc = (int)e;
+    e = cudaStreamSynchronize(h->st);
+    if (rc == CHASE_OK && e != cudaSuccess) rc = (int)e;
+    return rc;
+}
+
+int chase_filter_host_close(void *handle) {
+    if (!handle) return CHASE_ERR_ARG;
+    HostFilter *h = (HostFilter *)handle;
+    const cudaError_t e = cudaSetDevice(h->device);
+    host_filter_destroy(h);
+    return (int)e;
 }
 
 }  // extern "C"

@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include <vector>
 #include "chase_filter.h"
+#include "chase_filter_bench.h"
 
 namespace chase {
 
@@ -53,6 +54,9 @@ struct StepPlan {
 };
 // Bytes of device scratch the stream-K CTAs need (flags + one partial accumulator tile per CTA).
 size_t dmma_sk_scratch_bytes();
+// Frees the library's cached stream-K buffers (those launches without a caller workspace take); cudaErrorNotReady
+// if a launch on another host thread holds one right now.
+cudaError_t dmma_sk_cache_clear();
 void dmma_step_plan(int64_t N, int64_t n, chase_dtype_t dtype, int sms, StepPlan *out);
 
 // A plan holds the three tensor maps (H, and both vector buffers) of one chase_filter call.
@@ -91,7 +95,7 @@ cudaError_t dmma_plan_create_panel(DmmaPlan *plan, chase_dtype_t dtype, const vo
 cudaError_t dmma_launch_step(DmmaPlan *plan, int src, int64_t s, double alpha, double beta,
                              double c, int use_beta, cudaStream_t stream, const double *c_col = nullptr);
 
-// tcgen05 3xTF32 kernels (CHASE_C64 with N % 2 == 0, CHASE_F32 with N % 4 == 0).
+// tcgen05 split-precision CTA-pair kernels (CHASE_C64 with N % 2 == 0, CHASE_F32 with N % 4 == 0).
 struct Tf32Plan {
     alignas(64) unsigned char tmap_A[128];      // H viewed K-major (Hermitian: row m along k = conj of column m)
     alignas(64) unsigned char tmap_B[2][128];   // [0]: the caller's V, [1]: the workspace W
@@ -99,7 +103,6 @@ struct Tf32Plan {
     int64_t N, ncols;
     void *buf[2];
     void *sync_ctr;                             // 4-byte counter of the producers' soft grid barrier
-    int pair;                                   // 1: CTA-pair kernel (cta_group::2, 256-row tiles), 0: single-CTA kernel
     int mixed;                                  // 1: TF32 hi*hi + one BF16 MMA for both cross terms, 0: classic 3xTF32
 };
 bool tf32_supported(int64_t N, int64_t ncols, chase_dtype_t dtype);

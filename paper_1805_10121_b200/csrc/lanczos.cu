@@ -302,7 +302,6 @@ cudaError_t lanczos_ritz_vectors(const void *workspace, int64_t N, int nvec, int
     cudaError_t err;
     if ((err = cudaMemcpyAsync(d_S, S.data(), S.size() * sizeof(double), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return err;
     if ((err = cudaMemcpyAsync(d_dst, dst_cols, (size_t)cnt * sizeof(int64_t), cudaMemcpyHostToDevice, stream)) != cudaSuccess) return err;
-    if ((err = cudaStreamSynchronize(stream)) != cudaSuccess) return err;   // S is a local: consumed before return
     const dim3 grid((unsigned)((N + kBlock - 1) / kBlock), (unsigned)cnt);
     switch (dtype) {
         case CHASE_F32:  lz_ritz_vectors<float><<<grid, kBlock, 0, stream>>>((const float *)workspace, N, nvec, run, k, d_S, (float *)Vhat, d_dst); break;
@@ -311,7 +310,10 @@ cudaError_t lanczos_ritz_vectors(const void *workspace, int64_t N, int nvec, int
         default:         lz_ritz_vectors<double2><<<grid, kBlock, 0, stream>>>((const double2 *)workspace, N, nvec, run, k, d_S, (double2 *)Vhat, d_dst); break;
     }
     count_launch();
-    return cudaGetLastError();
+    if ((err = cudaGetLastError()) != cudaSuccess) return err;
+    // The documented contract: Vhat is complete when this returns.  (S is pageable, so the runtime staged it
+    // before cudaMemcpyAsync returned; the caller's dst_cols may be pinned and is only safe to reuse from here on.)
+    return cudaStreamSynchronize(stream);
 }
 
 bool lanczos_ritz(int k, const double *alpha, const double *beta, std::vector<double> &lam, std::vector<double> &w) {

@@ -765,12 +765,7 @@ void make_plan(int64_t M, int64_t N, int64_t n, int sms, bool allow_sk, StepPlan
     constexpr int WARPS_N = kConsumerWarps / C::WARPS_M;
     constexpr int Q = 8 * WARPS_N;                            // columns per quarter tile
     constexpr int QPT = C::BN / Q;                            // quarters per full tile (4)
-    // quarter slabs a stream-K CTA should at least get (CHASE_SK_MIN_WORK overrides; 0 disables stream-K: experiments)
-    static const int kMinWork = [] {
-        const char *env = std::getenv("CHASE_SK_MIN_WORK");
-        return env && env[0] ? std::atoi(env) : 4;
-    }();
-    if (kMinWork <= 0) allow_sk = false;
+    constexpr int kMinWork = 4;                               // quarter slabs a stream-K CTA should at least get
     const int KT = (int)((N + C::BK - 1) / C::BK);
     const int tiles_m = (int)((M + C::BM - 1) / C::BM);
     sms = std::max(1, std::min(sms, kMaxSkCtas));
@@ -913,7 +908,11 @@ struct SkSlot {
 std::mutex g_sk_mu;
 std::vector<SkSlot> g_sk_slots;
 
-cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch, unsigned *sync_base, unsigned sync_arrivals) {
+// `stream`: the stream the launch that takes the buffer goes to.  A fresh buffer's flag block is zeroed ON THAT
+// STREAM: a plain cudaMemset runs on the legacy default stream, which a non-blocking stream (chase_filter_host's,
+// any torch side stream) does not wait for, so the kernel could otherwise meet uninitialised flags.
+cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch, unsigned *sync_base, unsigned sync_arrivals,
+                             cudaStream_t stream) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -934,7 +933,7 @@ cudaError_t sk_cache_acquire(int *slot, void **ptr, uint32_t *epoch, unsigned *s
     sl.dev = dev; sl.held = true; sl.epoch = 1; sl.sync_count = sync_arrivals;
     *sync_base = 0;
     if ((e = cudaMalloc(&sl.ptr, dmma_sk_scratch_bytes())) != cudaSuccess) return e;
-    if ((e = cudaMemset(sl.ptr, 0, kSkFlagBytes)) != cudaSuccess ||
+    if ((e = cudaMemsetAsync(sl.ptr, 0, kSkFlagBytes, stream)) != cudaSuccess ||
         (e = cudaEventCreateWithFlags(&sl.ev, cudaEventDisableTiming)) != cudaSuccess) {
         cudaFree(sl.ptr);
         return e;
@@ -956,6 +955,27 @@ cudaError_t sk_cache_release(int slot, cudaStream_t stream) {
     const cudaError_t e = cudaEventRecord(sl.ev, stream);
     sl.held = false;
     return e;
+}
+
+// Gives the cached buffers back to the driver (chase_scratch_cache_release): waits for the launch each one last
+// served, frees it, forgets it.  A buffer some host thread holds at this moment stays.
+cudaError_t sk_cache_clear() {
+    std::lock_guard<std::mutex> lock(g_sk_mu);
+    cudaError_t first = cudaSuccess;
+    for (SkSlot &sl : g_sk_slots) {
+        if (sl.held) {
+            // indices of held slots must stay valid for their sk_cache_release: only a cache without held slots shrinks
+            return cudaErrorNotReady;
+        }
+    }
+    for (SkSlot &sl : g_sk_slots) {
+        cudaError_t e = cudaEventSynchronize(sl.ev);
+        if (e == cudaSuccess) e = cudaFree(sl.ptr);
+        const cudaError_t e2 = cudaEventDestroy(sl.ev);
+        if (first == cudaSuccess) first = e != cudaSuccess ? e : e2;
+    }
+    g_sk_slots.clear();
+    return first;
 }
 
 template <bool CPLX>
@@ -995,7 +1015,7 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
     cudaError_t e;
     if (pl.sk_ctas > 0) {
         if (!scratch) {
-            if ((e = sk_cache_acquire(&cache_slot, (void **)&scratch, &epoch, &sync_base, sync_arrivals)) != cudaSuccess)
+            if ((e = sk_cache_acquire(&cache_slot, (void **)&scratch, &epoch, &sync_base, sync_arrivals, stream)) != cudaSuccess)
                 return e;
         } else {
             if (plan->sk_epoch == 0) {                                     // flags and counter start at 0, epochs at 1
@@ -1065,6 +1085,8 @@ cudaError_t launch(DmmaPlan *plan, int src, int64_t s, double alpha, double beta
 }  // namespace
 
 size_t dmma_sk_scratch_bytes() { return kSkFlagBytes + (size_t)kMaxSkCtas * kPartBytes; }
+
+cudaError_t dmma_sk_cache_clear() { return sk_cache_clear(); }
 
 void dmma_step_plan(int64_t N, int64_t n, chase_dtype_t dtype, int sms, StepPlan *out) {
     if (dtype == CHASE_C128) make_plan<true>(N, N, n, sms, true, *out);

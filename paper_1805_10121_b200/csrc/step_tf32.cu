@@ -1,35 +1,39 @@
-// tcgen05 (5th-gen tensor core) step kernel for float32 / complex64: 3xTF32 split products with
+// tcgen05 (5th-gen tensor core) step kernel for float32 / complex64: split-precision products on CTA pairs with
 // FP32 accumulation in TMEM.
 //
 //   Y[:, j] <- alpha * (H X[:, j] - c X[:, j]) + beta * Y[:, j]     (Alg. 4 l.4 / l.9; Eq. 7)
 //
-// Every fp32 operand x is split as x = hi + lo, hi = x with the low 13 mantissa bits cleared
-// (what kind::tf32 reads from an fp32 word), lo = x - hi (exact in fp32).  The product is
-// evaluated as hi*lo + lo*hi + hi*hi (lo*lo ~ 2^-22 relative is dropped): three tcgen05.mma per
-// k-slice into ONE fp32 accumulator in tensor memory, which restores fp32-level accuracy (plain
-// single-pass TF32, 2^-11 per operand, would not meet the 1e-4 bound).
+// ONE kernel: step_tf32_pair_kernel<CPLX, MIXED>, 512 threads per CTA, two CTAs of a cluster (the two SMs of a
+// TPC) on one 256 x 256 tile through tcgen05.mma.cta_group::2 (the section "CTA-pair variant" below has the
+// roles, the rings and the barriers).
 //
-// Only the fp32 data itself crosses L2: TMA brings the raw H and X tiles (they serve as the hi
-// operands, the tensor core ignores the low mantissa bits) and two converter warps derive the lo
-// tiles -- and for complex64 the rotated tile -i X -- in shared memory.  The split is element-wise
-// and the rotation stays inside a 16-byte chunk, so both are oblivious of the 64-byte swizzle.
+// Every fp32 operand x is split as x = hi + lo, hi = x with the low 13 mantissa bits cleared (what kind::tf32
+// reads from an fp32 word), lo = x - hi (exact in fp32).  A product is hi*hi + (hi*lo + lo*hi); lo*lo ~ 2^-22
+// relative is dropped.  hi*hi is a kind::tf32 MMA on the raw tiles.  The cross terms are
+//   MIXED = true (default): ONE kind::f16 MMA on BF16 "pair tiles" over a doubled K (pack_pair below): 2 MMA units
+//                           per product, error vs an FP64 evaluation ~2e-5 at degree 16;
+//   MIXED = false (CHASE_TF32_MIXED=0): two more kind::tf32 MMAs on lo tiles -- classic 3xTF32, 3 units.
+// All of them accumulate into one fp32 accumulator in tensor memory; plain single-pass TF32 (2^-11 per operand)
+// would not meet the 1e-4 bound.
+//
+// Only the fp32 data itself crosses L2: TMA brings the raw H and X tiles (they serve as the hi operands, the tensor
+// core ignores the low mantissa bits) and the converter warps derive the second tiles (lo or BF16 pair) -- and for
+// complex64 the rotated tile -i X -- in shared memory.  The split is element-wise and the rotation stays inside a
+// 16-byte chunk, so both are oblivious of the 64-byte swizzle.
 //
 // Both operands are K-major.  For A this uses that H is Hermitian (reading G9): row m of
 // H along k is the conjugate of column m, which is contiguous in the column-major storage.
-//   float32:   A[m][k] = H[k][m] (column m read along k); B = X as stored; D = 128 rows x 256 columns.
+//   float32:   A[m][k] = H[k][m] (column m read along k); B = X as stored.
 //   complex64: a REAL GEMM over the interleaved index kk = 2k + {0, 1}:
 //     A2[m][kk]  = column m of H as floats    = (Re A[m,k], -Im A[m,k])      (conjugate of H[k,m])
 //     B1[kk][j]  = column j of X as floats    = (Re x, Im x)
 //     B2[kk][j]  = column j of -i X           = (Im x, -Re x)
-//     A2 . B1 = Re(A x),  A2 . B2 = Im(A x):  D = 128 complex rows x [128 Re | 128 Im] columns.
+//     A2 . B1 = Re(A x),  A2 . B2 = Im(A x):  D = complex rows x [128 Re | 128 Im] columns.
 //
-// Warp roles (384 threads, 1 persistent CTA / SM): warp 0 = TMA producer (one lane), warp 1 = TMEM
-// allocator + MMA issuer (one lane), warps 2-3 = converters, warps 4-11 = accumulator/epilogue warps
-// (TMEM lane quarter = warp % 4, column half = (warp-4)/4).  The MMA issuer accumulates CHUNK stages
-// into one of two TMEM buffers; the accumulator warps add each finished chunk into fp32 registers
-// (round to nearest) while the tensor core fills the other buffer, then run the fused epilogue.
-// Shared-memory operand tiles are the canonical K-major SWIZZLE_64B UMMA layout written directly
-// by TMA: [row][16 floats of k] (64-byte rows, 8-row groups 512 B apart); one UMMA consumes 8 k.
+// The MMA issuer accumulates CHUNK stages into one of two TMEM buffers; the accumulator warps add each finished
+// chunk into fp32 registers (round to nearest) while the tensor core fills the other buffer, then run the fused
+// epilogue.  Shared-memory operand tiles are the canonical K-major SWIZZLE_64B UMMA layout written directly by
+// TMA: [row][16 floats of k] (64-byte rows, 8-row groups 512 B apart); one TF32 UMMA consumes 8 k.
 #include <cuda.h>
 
 #include <algorithm>
@@ -41,22 +45,16 @@
 namespace chase {
 namespace {
 
-constexpr int kConvWarps = 2;      // converter warps (lo parts and -i X, in shared memory)
 constexpr int kFirstAccWarp = 4;   // multiple of 4: TMEM lane quarter = warp % 4
 constexpr int kAccWarps = 8;       // accumulator / epilogue warps: 4 TMEM lane quarters x 2 column halves
-constexpr int kThreads = (kFirstAccWarp + kAccWarps) * 32;
 constexpr int KS = 16;            // floats of k per pipeline stage (two UMMA K = 8 slices)
 constexpr int TM = 128;           // (complex or real) rows per CTA tile = TMEM lanes
 constexpr int TN = 256;           // real B columns per CTA tile = TMEM columns
-constexpr int STAGES = 4;
 #ifndef TF32_CHUNK
 #define TF32_CHUNK 8
 #endif
 constexpr int CHUNK = TF32_CHUNK;            // pipeline stages accumulated in TMEM before the sum moves to registers
 constexpr int A_BYTES = TM * KS * 4;          // 8 KB
-constexpr int B_BYTES = TN * KS * 4;          // 16 KB
-constexpr int STAGE_BYTES = 2 * A_BYTES + 2 * B_BYTES;   // hi + lo of both: 48 KB
-constexpr int SMEM_TOTAL = STAGES * STAGE_BYTES + 1024 + 256;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -64,9 +62,6 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     uint32_t done;
@@ -110,46 +105,6 @@ __device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap *map, int c0, 
 __device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes, uint32_t layout) {
     return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | ((uint64_t)1 << 46) | ((uint64_t)layout << 61);
-}
-// Instruction descriptor, kind::tf32: D fp32 (bits 4-5 = 1), A/B TF32 (bits 7-9, 10-12 = 2),
-// A and B K-major (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28.
-constexpr uint32_t kInstrDesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TN >> 3) << 17) |
-                                ((uint32_t)(TM >> 4) << 24);
-
-__device__ __forceinline__ void umma_tf32(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n.reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n}\n"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDesc), "r"(accumulate) : "memory");
-}
-// kind::f16 with BF16 operands (a_format = b_format = 1), fp32 accumulate: same tile shape, K = 16 per instruction
-constexpr uint32_t kInstrDescBf16 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) |
-                                    ((uint32_t)(TM >> 4) << 24);
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n.reg .pred p;\n"
-        "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n"
-        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(kInstrDescBf16), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
-    uint32_t r[32];
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr) : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-    for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
     uint32_t r[16];
@@ -250,236 +205,6 @@ __device__ __forceinline__ bool soft_grid_sync(unsigned *ctr, unsigned target) {
 // X column panels in L2).  The resident CTAs only share those panels if they walk along k TOGETHER: the
 // L2 holds ~18 pipeline stages of the union stream, a tile lasts ~7500 stages.  So the producers meet at
 // a soft barrier at the start of every tile and every kSyncStages stages.
-template <bool CPLX>
-__global__ void __launch_bounds__(kThreads, 1)
-step_tf32_kernel(const __grid_constant__ CUtensorMap tmapA, const __grid_constant__ CUtensorMap tmapB,
-                 const Tf32Params p) {
-    constexpr int COLS = CPLX ? TN / 2 : TN;      // (complex or real) columns per tile
-    extern __shared__ __align__(1024) unsigned char smem_raw[];
-    unsigned char *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-    const uint32_t smem_base = smem_u32(smem);
-    const uint32_t bar_base = smem_base + STAGES * STAGE_BYTES;   // full[S], empty[S], conv[S], tfull[2], tempty[2], tmem slot
-    const uint32_t bar_conv = bar_base + 8 * (2 * STAGES);
-    const uint32_t bar_tfull = bar_base + 8 * (3 * STAGES);
-    const uint32_t bar_tempty = bar_base + 8 * (3 * STAGES + 2);
-    const uint32_t tmem_slot = bar_base + 8 * (3 * STAGES + 4);
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int total_tiles = p.tiles_m * p.tiles_n;
-    const int KT = (int)((p.KF + KS - 1) / KS);          // pipeline stages over k, per tile
-    const int NCH = (KT + CHUNK - 1) / CHUNK;            // TMEM accumulation chunks, per tile
-
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) {
-            mbar_init(bar_base + 8 * s, 1);              // full: producer's expect_tx arrive
-            mbar_init(bar_base + 8 * (STAGES + s), 1);   // empty: one tcgen05.commit arrive
-            mbar_init(bar_conv + 8 * s, kConvWarps);     // conv: lo / rot tiles written by every converter warp
-        }
-        for (int b = 0; b < 2; ++b) {
-            mbar_init(bar_tfull + 8 * b, 1);             // chunk accumulator complete (tcgen05.commit)
-            mbar_init(bar_tempty + 8 * b, kAccWarps);    // chunk accumulator drained by every accumulator warp
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (warp == 1) {   // all of TMEM: two 256-column fp32 accumulators (ping-pong between chunks)
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "r"(2 * TN) : "memory");
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    uint32_t tmem_base;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot) : "memory");
-
-    if (warp == 0) {
-        // ------------------------------------------------------------------ TMA producer
-        if (lane == 0) {
-            const int syncs_per_tile = (KT + kSyncStages - 1) / kSyncStages;
-            unsigned it = 0;                                  // stages filled so far (all tiles)
-            unsigned *sync_ctr = p.sync_ctr;
-            int round = 0;
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++round) {
-                int tile_m, tile_n;
-                tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
-                const int m0 = tile_m * TM, n0 = tile_n * COLS;
-                const unsigned active = (unsigned)min((int)gridDim.x, total_tiles - round * (int)gridDim.x);
-                const unsigned sync_base = (unsigned)round * gridDim.x * (unsigned)syncs_per_tile;
-                for (int kt = 0; kt < KT; ++kt, ++it) {
-                    if (sync_ctr && kt % kSyncStages == 0 &&
-                        !soft_grid_sync(sync_ctr, sync_base + active * (unsigned)(kt / kSyncStages + 1)))
-                        sync_ctr = nullptr;
-                    const int s = it % STAGES;
-                    const uint32_t full = bar_base + 8 * s, empty = bar_base + 8 * (STAGES + s);
-                    if (it >= STAGES) mbar_wait(empty, ((it / STAGES) - 1) & 1);
-                    const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
-                    const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
-                    const int k0 = kt * KS;
-                    // raw fp32 tiles only: 128 columns of H and 128 (complex) / 256 (real) columns of X, 16 floats of k
-                    mbar_expect_tx(full, A_BYTES + (CPLX ? B_BYTES / 2 : B_BYTES));
-                    tma_load_2d(sa_hi, &tmapA, full, k0, m0);
-                    tma_load_2d(sb_hi, &tmapB, full, k0, p.col0 + n0);
-                    (void)sa_lo; (void)sb_lo;
-                }
-            }
-        }
-    } else if (warp == 1) {
-        // ------------------------------------------------------------------ MMA issuer
-        if (lane == 0) {
-            unsigned it = 0, gc = 0;                          // stages consumed / chunks issued so far (all tiles)
-            for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-                int kt = 0;
-                for (int ch = 0; ch < NCH; ++ch, ++gc) {
-                    const int b = gc & 1;
-                    if (gc >= 2) {   // the accumulator warps must have drained this buffer's previous chunk
-                        mbar_wait(bar_tempty + 8 * b, ((gc >> 1) - 1) & 1);
-                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                    }
-                    const uint32_t d = tmem_base + b * TN;
-                    const int kt_end = min(KT, kt + CHUNK);
-                    for (bool first = true; kt < kt_end; ++kt, ++it) {
-                        const int s = it % STAGES;
-                        mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);      // TMA tiles landed
-                        mbar_wait(bar_conv + 8 * s, (it / STAGES) & 1);      // lo / rot tiles written
-                        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                        const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
-                        const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
-#pragma unroll
-                        for (int ks = 0; ks < KS / 8; ++ks) {
-                            // K-major SWIZZLE_64B: 8-row groups 512 B apart; the 8-k slice ks starts 32 B into the row
-                            const uint64_t ah = umma_desc(sa_hi + ks * 32, 16, 512, 4);
-                            const uint64_t al = umma_desc(sa_lo + ks * 32, 16, 512, 4);
-                            const uint64_t bh = umma_desc(sb_hi + ks * 32, 16, 512, 4);
-                            const uint64_t bl = umma_desc(sb_lo + ks * 32, 16, 512, 4);
-                            if (p.mixed) {
-                                umma_bf16(d, al, bl, first ? 0u : 1u);    // x_b * lo_b + lo_b * x_b (pair tiles, K = 16)
-                            } else {
-                                umma_tf32(d, ah, bl, first ? 0u : 1u);    // hi * lo  (first MMA of a chunk overwrites)
-                                umma_tf32(d, al, bh, 1u);                 // lo * hi
-                            }
-                            umma_tf32(d, ah, bh, 1u);                     // hi * hi
-                            first = false;
-                        }
-                        umma_commit(bar_base + 8 * (STAGES + s));   // frees the smem stage when these MMAs retire
-                    }
-                    umma_commit(bar_tfull + 8 * b);                  // this chunk's accumulator is complete
-                }
-            }
-        }
-    } else if (warp < 2 + kConvWarps) {
-        // ------------------------------------------------------------------ converter warps
-        // Stage layout: [A raw | A lo | B hi (complex: X raw, -iX) | B lo (complex: X lo, (-iX) lo)].
-        constexpr int CT = kConvWarps * 32;
-        const int ct = threadIdx.x - 64;
-        unsigned it = 0;
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            for (int kt = 0; kt < KT; ++kt, ++it) {
-                const int s = it % STAGES;
-                mbar_wait(bar_base + 8 * s, (it / STAGES) & 1);
-                const uint32_t sa_hi = smem_base + s * STAGE_BYTES, sa_lo = sa_hi + A_BYTES;
-                const uint32_t sb_hi = sa_lo + A_BYTES, sb_lo = sb_hi + B_BYTES;
-                {
-                    // all loads of a tile first (independent, pipelined through the LSU), then the stores
-                    constexpr int NA = A_BYTES / 16 / CT;
-                    float4 va[NA];
-#pragma unroll
-                    for (int i = 0; i < NA; ++i) va[i] = lds128(sa_hi + (uint32_t)(ct + i * CT) * 16);
-                    if (CPLX) {
-                        constexpr int NB = B_BYTES / 2 / 16 / CT;
-                        float4 vb[NB];
-#pragma unroll
-                        for (int i = 0; i < NB; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
-#pragma unroll
-                        for (int i = 0; i < NA; ++i)
-                            sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, second_tile<false>(va[i], p.mixed));
-#pragma unroll
-                        for (int i = 0; i < NB; ++i) {
-                            const uint32_t off = (uint32_t)(ct + i * CT) * 16;
-                            const float4 r = rot_mi(vb[i]);            // lo(-iX) = -i lo(X): the split is element-wise
-                            sts128(sb_lo + off, second_tile<true>(vb[i], p.mixed));
-                            sts128(sb_hi + B_BYTES / 2 + off, r);
-                            sts128(sb_lo + B_BYTES / 2 + off, second_tile<true>(r, p.mixed));
-                        }
-                    } else {
-                        constexpr int NB = B_BYTES / 16 / CT;
-                        float4 vb[NB / 2];
-#pragma unroll
-                        for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + i * CT) * 16);
-#pragma unroll
-                        for (int i = 0; i < NA; ++i)
-                            sts128(sa_lo + (uint32_t)(ct + i * CT) * 16, second_tile<false>(va[i], p.mixed));
-#pragma unroll
-                        for (int i = 0; i < NB / 2; ++i)
-                            sts128(sb_lo + (uint32_t)(ct + i * CT) * 16, second_tile<true>(vb[i], p.mixed));
-#pragma unroll
-                        for (int i = 0; i < NB / 2; ++i) vb[i] = lds128(sb_hi + (uint32_t)(ct + (i + NB / 2) * CT) * 16);
-#pragma unroll
-                        for (int i = 0; i < NB / 2; ++i)
-                            sts128(sb_lo + (uint32_t)(ct + (i + NB / 2) * CT) * 16, second_tile<true>(vb[i], p.mixed));
-                    }
-                }
-                // generic-proxy writes -> visible to the tensor core's async-proxy reads
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_conv + 8 * s);
-            }
-        }
-    } else if (warp >= kFirstAccWarp) {
-        // ------------------------------------------------------------------ accumulator / epilogue warps
-        // The tensor core's fp32 accumulation rounds toward zero, a bias that grows with the length
-        // of the accumulation chain; so the chain is cut into chunks of CHUNK stages, and the chunk
-        // sums are added here in registers with round-to-nearest.
-        const int quarter = warp & 3;                       // TMEM lanes this warp may access
-        const int half = (warp - kFirstAccWarp) >> 2;       // which 128 of the 256 accumulator columns
-        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + half * (TN / 2);
-        const float alpha = p.alpha, beta = p.beta;
-        unsigned gc = 0;                                     // chunks drained so far (all tiles)
-        for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-            int tile_m, tile_n;
-            tile_coords(tile, p.tiles_m, p.tiles_n, tile_m, tile_n);
-            const int m0 = tile_m * TM, n0 = tile_n * COLS;
-            float racc[TN / 2];
-#pragma unroll
-            for (int i = 0; i < TN / 2; ++i) racc[i] = 0.f;
-            for (int ch = 0; ch < NCH; ++ch, ++gc) {
-                const int b = gc & 1;
-                mbar_wait(bar_tfull + 8 * b, (gc >> 1) & 1);
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-                for (int j = 0; j < TN / 2 / 32; ++j) {
-                    float t[32];
-                    tmem_ld32(taddr + b * TN + j * 32, t);
-#pragma unroll
-                    for (int i = 0; i < 32; ++i) racc[j * 32 + i] += t[i];
-                }
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(bar_tempty + 8 * b);
-            }
-
-            const int64_t row = (int64_t)m0 + quarter * 32 + lane;
-            const bool row_ok = row < p.N;
-#pragma unroll
-            for (int i = 0; i < TN / 2; ++i) {
-                // complex: half 0 owns the real parts, half 1 the imaginary parts of columns n0 .. n0+127
-                const int col = CPLX ? n0 + i : n0 + half * (TN / 2) + i;
-                if (col < p.n && row_ok) {
-                    const float c = p.c_col ? (float)p.c_col[col] : p.c;
-                    const int64_t off = CPLX ? ((int64_t)col * p.N + row) * 2 + half : (int64_t)col * p.N + row;
-                    float y = alpha * (racc[i] - c * __ldcg(p.X + off));   // L2 only: see step_dmma.cu
-                    if (p.use_beta) y = fmaf(beta, __ldcg(p.Y + off), y);
-                    p.Y[off] = y;
-                }
-            }
-        }
-    }
-
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (warp == 1) {
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(2 * TN) : "memory");
-    }
-}
-
 // ---------------------------------------------------------------- CTA-pair variant (cta_group::2)
 // Two CTAs of a cluster (the two SMs of a TPC) share one 256 x 256 tile: tcgen05.mma.cta_group::2 with
 // M = 256 takes 128 rows of A from each CTA's shared memory and HALF of B (128 of the 256 real columns)
@@ -891,10 +616,8 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     static std::once_flag once;
     static cudaError_t attr_err = cudaSuccess;
     std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(step_tf32_kernel<CPLX>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_TOTAL);
-        if (attr_err == cudaSuccess)
-            attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX, true>,
-                                            cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_TOTAL);
+        attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX, true>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_TOTAL);
         if (attr_err == cudaSuccess)
             attr_err = cudaFuncSetAttribute(step_tf32_pair_kernel<CPLX, false>,
                                             cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM2_TOTAL);
@@ -913,8 +636,7 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
     p.KF = plan->N * FL;
     p.n = (int)n;
     p.col0 = (int)s;
-    const bool pair = plan->pair != 0;
-    p.tiles_m = pair ? (int)((plan->N + 2 * TM - 1) / (2 * TM)) : (int)((plan->N + TM - 1) / TM);
+    p.tiles_m = (int)((plan->N + 2 * TM - 1) / (2 * TM));           // 256 rows per CTA pair
     p.tiles_n = (int)((n + COLS - 1) / COLS);
     p.alpha = (float)alpha;
     p.beta = (float)beta;
@@ -928,20 +650,14 @@ cudaError_t launch(const Tf32Plan *plan, int src, int64_t s, double alpha, doubl
         cudaError_t e = cudaMemsetAsync(p.sync_ctr, 0, sizeof(unsigned), stream);
         if (e != cudaSuccess) return e;
     }
-    if (pair) {   // persistent CTA pairs: one cluster of 2 per TPC
-        const int grid = 2 * std::min(total_tiles, std::max(1, sm_count() / 2));
-        if (plan->mixed)
-            step_tf32_pair_kernel<CPLX, true><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
-                *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
-        else
-            step_tf32_pair_kernel<CPLX, false><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
-                *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
-        count_launch();
-        return cudaGetLastError();
-    }
-    const int grid = std::min(total_tiles, sm_count());      // persistent: one CTA per SM
-    step_tf32_kernel<CPLX><<<(unsigned)grid, kThreads, SMEM_TOTAL, stream>>>(
-        *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
+    // persistent CTA pairs: one cluster of 2 per TPC
+    const int grid = 2 * std::min(total_tiles, std::max(1, sm_count() / 2));
+    if (plan->mixed)
+        step_tf32_pair_kernel<CPLX, true><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
+            *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
+    else
+        step_tf32_pair_kernel<CPLX, false><<<(unsigned)grid, kThreads2, SMEM2_TOTAL, stream>>>(
+            *(const CUtensorMap *)plan->tmap_A, *(const CUtensorMap *)plan->tmap_B[src], p);
     count_launch();
     return cudaGetLastError();
 }
@@ -968,15 +684,12 @@ cudaError_t tf32_plan_create(Tf32Plan *plan, chase_dtype_t dtype, const void *H,
     plan->buf[0] = V;
     plan->buf[1] = workspace;
     plan->sync_ctr = (workspace && vb) ? (char *)workspace + vb : nullptr;
-    // CTA pairs (cta_group::2) unless CHASE_TF32_PAIR=0 asks for the single-CTA kernel (experiments / fallback)
-    const char *pair_env = std::getenv("CHASE_TF32_PAIR");
-    plan->pair = !(pair_env && pair_env[0] == '0');
     // cross terms hi*lo + lo*hi as ONE BF16 MMA (2 MMA units per product) unless CHASE_TF32_MIXED=0 (classic 3xTF32)
     const char *mixed_env = std::getenv("CHASE_TF32_MIXED");
     plan->mixed = !(mixed_env && mixed_env[0] == '0');
     cudaError_t e;
     if ((e = encode_kmajor((CUtensorMap *)plan->tmap_A, H, KF, N, TM)) != cudaSuccess) return e;
-    const int b_box = plan->pair ? TN / 2 : (cplx ? TN / 2 : TN);      // B columns one TMA box brings
+    const int b_box = TN / 2;                                          // B columns one TMA box brings (one CTA's half)
     for (int i = 0; i < 2; ++i)
         if (plan->buf[i] &&
             (e = encode_kmajor((CUtensorMap *)plan->tmap_B[i], plan->buf[i], KF, ncols, b_box)) != cudaSuccess)

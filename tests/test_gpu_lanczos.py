@@ -67,15 +67,18 @@ def test_ritz_vectors_match_oracle_and_land_in_the_chosen_columns(dtype, N):
     Vhat0 = W.gaussian_colmajor(N, 2 * k, dtype, seed=99)
     Vhat = _dev(Vhat0)
     dst = list(range(1, 2 * k, 2))                          # odd columns: interspersed with the random ones
-    vals = pkg.chase_lanczos_ritz_vectors(ws, N, dtype, alpha, beta, 1, mu_ne, Vhat, dst)
     torch.cuda.synchronize()
+    # on a non-blocking side stream and with NO synchronisation of ours afterwards: the call itself promises that
+    # Vhat is complete on return (the read below runs on the default stream, which does not wait for `side`)
+    side = torch.cuda.Stream()
+    vals = pkg.chase_lanczos_ritz_vectors(ws, N, dtype, alpha, beta, 1, mu_ne, Vhat, dst, stream=side)
+    got = Vhat.cpu().numpy()
     Hn, Vn = w.H.numpy(), w.V0.numpy()
     a_ref, b_ref, U_ref, _ = OL.lanczos(Hn, Vn[:, 1], k)
     lam_ref, X_ref, _ = OL.ritz_vectors(U_ref, a_ref, b_ref, mu_ne)
     assert 0 < len(lam_ref) < k and len(vals) == len(lam_ref)
     tol = 1e-9 if dtype in (torch.complex128, torch.float64) else 2e-3
     np.testing.assert_allclose(vals, lam_ref, atol=tol)
-    got = Vhat.cpu().numpy()
     for i in range(len(vals)):
         assert np.linalg.norm(got[:, dst[i]] - X_ref[:, i]) <= tol * 10, i
     untouched = [c for c in range(2 * k) if c not in dst[: len(vals)]]

@@ -226,6 +226,30 @@ def test_host_entry_point(cfg, N, ncols, dtype):
     assert_parity(V.numpy(), run_oracle(w), w.dtype)
 
 
+@pytest.mark.parametrize("cfg,N,dtype", [(4, 1032, None), (5, 768, None), (2, 203, torch.float64)])
+def test_host_handle_keeps_H_resident(cfg, N, dtype):
+    """chase_filter_host_open / _run / _close: H goes up once, then several runs with different widths, degrees
+    and bounds on the same handle, each equal to the oracle; degree-0 columns are never transferred."""
+    wide = W.make_config(cfg, N=N, ncols=96, dtype=dtype)
+    with pkg.HostFilter(wide.H, max_ncols=96, device=0) as hf:
+        for ncols, seed in ((96, 1), (40, 2), (96, 3), (7, 4)):
+            w = W.make_config(cfg, N=N, ncols=ncols, dtype=dtype)        # same seeded H for every ncols
+            assert torch.equal(w.H, wide.H)
+            deg = w.degrees.clone()
+            if seed == 3:
+                deg[:5] = 0
+                deg[5:9] = 3                                               # untouched and odd-degree columns
+                deg, _ = torch.sort(deg)
+            V = W.as_colmajor(w.V0.clone())
+            hf.run(V, deg, w.a, w.b - 0.01 * seed, w.lambda1)
+            ref = oracle.chase_filter(w.H.numpy(), w.V0.numpy(), deg.numpy(), w.a, w.b - 0.01 * seed, w.lambda1)
+            assert_parity(V.numpy(), ref, w.dtype)
+        with pytest.raises(pkg.ChaseFilterError):
+            hf.run(W.as_colmajor(torch.zeros(N, 97, dtype=wide.dtype)), [2] * 97, wide.a, wide.b, wide.lambda1)
+    with pytest.raises(ValueError):
+        hf.run(W.as_colmajor(wide.V0.clone()), wide.degrees, wide.a, wide.b, wide.lambda1)     # closed
+
+
 def test_peak_probes_run():
     dfma = pkg.chase_fp64_peak_probe(0, 2048)
     dmma = pkg.chase_fp64_peak_probe(1, 2048)

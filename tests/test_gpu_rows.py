@@ -47,6 +47,28 @@ def test_hemm_rows_with_peer_pushes(dtype, N, n, world, align):
         assert rel_fro(Ys[q].cpu().numpy(), ref) <= 1e-12, q
 
 
+def test_hemm_rows_on_side_stream_with_cold_scratch_cache():
+    """The row-sharded HEMM takes its stream-K scratch from the library's cache; a fresh buffer must be zeroed on
+    the launching (non-blocking) stream, not on the legacy default stream."""
+    dtype, N, n, world = torch.complex128, 520, 77, 3
+    H = W.hermitian_gaussian_ensemble(N, dtype, seed=84)
+    X = W.gaussian_colmajor(N, n, dtype, seed=85)
+    parts, Hb = _row_blocks(H, world, 128)
+    Xd = _dev(X)
+    ref = oracle.hemm(H.numpy(), X.numpy(), None)
+    torch.cuda.synchronize()
+    for _ in range(3):
+        pkg.chase_scratch_cache_release()
+        st = torch.cuda.Stream()
+        Yd = W.empty_colmajor(N, n, dtype, DEV)
+        Yd.fill_(float("nan"))
+        torch.cuda.synchronize()
+        for r, (row0, nrows) in enumerate(parts):
+            pkg.chase_hemm_rows(Hb[r], row0, Xd, Yd, stream=st)
+        st.synchronize()
+        assert rel_fro(Yd.cpu().numpy(), ref) <= 1e-12
+
+
 @pytest.mark.parametrize("dtype,N,n,world", [(torch.complex128, 520, 77, 3), (torch.float64, 1040, 150, 2)])
 def test_filter_emulated_ranks_step_by_step(dtype, N, n, world):
     """Alg. 4 driven from the host plan (chase_filter_scalars / _schedule) with one chase_hemm_rows per
@@ -87,6 +109,37 @@ def test_filter_rows_single_rank_equals_plain_filter(with_flags):
         assert seq == 5 + 1 + m_max and int(flags.cpu()[0]) == seq      # one barrier on entry, one per step
         pkg.chase_rows_status(flags, 1)                                 # no barrier timed out
         assert int(flags.cpu()[1]) == 0
+
+
+def test_host_barrier_exception_is_not_swallowed():
+    """A host barrier that raises (peer died, gloo timeout) must surface as that exception, at once -- not as a
+    success that sends the run into the wait kernel's 30 s timeout."""
+    import time
+    w = W.make_config(4, N=520, ncols=24)
+    H, V = _dev(w.H), _dev(w.V0)
+    ws = torch.empty(pkg.chase_filter_workspace_bytes(w.N, w.ncols, w.dtype), dtype=torch.uint8, device=DEV)
+    flags = torch.zeros(2, dtype=torch.int32, device=DEV)
+    calls = []
+
+    def barrier():
+        calls.append(1)
+        if len(calls) == 2:
+            raise RuntimeError("peer died")
+        return 0
+
+    t0 = time.perf_counter()
+    with pytest.raises(RuntimeError, match="peer died"):
+        pkg.chase_filter_rows_ws(H, 0, V, w.degrees, w.a, w.b, w.lambda1, ws, rank=0, flags=flags,
+                                 peer_flags=[flags.data_ptr()], seq=0, host_barrier=barrier)
+    torch.cuda.synchronize()
+    assert len(calls) == 2 and time.perf_counter() - t0 < 5.0
+    # a barrier that merely REPORTS failure still maps to CHASE_ERR_TIMEOUT
+    flags.zero_()
+    with pytest.raises(pkg.ChaseFilterError) as e:
+        pkg.chase_filter_rows_ws(H, 0, V, w.degrees, w.a, w.b, w.lambda1, ws, rank=0, flags=flags,
+                                 peer_flags=[flags.data_ptr()], seq=0, host_barrier=lambda: 3)
+    assert e.value.code == -7
+    torch.cuda.synchronize()
 
 
 def test_rows_rejects_unsupported_layouts():

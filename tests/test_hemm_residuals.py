@@ -102,3 +102,30 @@ def test_gpu_skinny_hemm_and_residuals(dtype, N, n):
     got = pkg.chase_residuals(Hd, Xd, ritz).cpu().numpy()
     np.testing.assert_allclose(got, oracle.residuals(H.numpy(), X.numpy(), ritz), rtol=10 * tol)
     assert torch.equal(Xd.cpu(), X) and torch.equal(Hd.cpu(), H)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype,N,n", [(torch.complex128, 520, 77), (torch.float64, 1040, 150)])
+def test_gpu_hemm_on_side_stream_with_cold_scratch_cache(dtype, N, n):
+    """chase_hemm brings no workspace: on the FP64 tensor path its stream-K flags live in a cached buffer the
+    library allocates on first use.  That buffer must be zeroed on the LAUNCHING stream -- a non-blocking
+    side stream does not wait for the legacy default stream -- so: empty the cache, launch on a fresh
+    torch stream, several times over."""
+    H = W.hermitian_gaussian_ensemble(N, dtype, seed=75)
+    X = W.gaussian_colmajor(N, n, dtype, seed=76)
+    Hd, Xd = _dev(H), _dev(X)
+    ref = oracle.hemm(H.numpy(), X.numpy(), None)
+    torch.cuda.synchronize()
+    for _ in range(4):
+        pkg.chase_scratch_cache_release()
+        st = torch.cuda.Stream()
+        Yd = W.empty_colmajor(N, n, dtype, "cuda")
+        Yd.fill_(float("nan"))
+        torch.cuda.synchronize()
+        with torch.cuda.stream(st):
+            pkg.chase_hemm(Hd, Xd, Yd, stream=st)
+            pkg.chase_hemm(Hd, Xd, Yd, alpha=1.0, beta=0.0, stream=st)      # warm slot, next epoch
+        st.synchronize()
+        assert rel_fro(Yd.cpu().numpy(), ref) <= 1e-12
+    pkg.chase_scratch_cache_release()
+    pkg.chase_scratch_cache_release()                                        # empty cache: a no-op

@@ -17,10 +17,15 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def test_library_exports_every_declared_symbol():
-    header = open(os.path.join(ROOT, "include", "chase_filter.h")).read()
-    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(chase_[a-z0-9_]+)\s*\(", header))
+    declared = set()
+    for name in sorted(os.listdir(os.path.join(ROOT, "include"))):       # product ABI + the bench/test hooks
+        header = open(os.path.join(ROOT, "include", name)).read()
+        header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+        declared |= set(re.findall(r"\b(chase_[a-z0-9_]+)\s*\(", header))
     assert declared == set(binding.EXPORTS)
+    product = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "chase_filter.h")).read(), flags=re.S)
+    for hook in ("chase_fp64_peak_probe", "chase_filter_launch_count", "chase_filter_step_plan"):
+        assert hook not in product            # hooks live in chase_filter_bench.h, not in the product header
     lib = ctypes.CDLL(pkg.lib_path())
     for name in declared:
         assert hasattr(lib, name), name
@@ -309,3 +314,13 @@ def test_parity_sample_plan_covers_every_degree_class_and_tile_edge():
         assert {63, 64, 65, 127, 128, 129} <= set(cols)
     assert W.parity_sample_columns([]) == []
     assert W.parity_sample_columns([2, 2, 4]) == [0, 1, 2]
+
+
+def test_host_handle_rejects_bad_arguments_before_any_cuda_call():
+    lib = pkg.load()
+    out = ctypes.c_void_p()
+    assert lib.chase_filter_host_open(None, 64, 8, binding.CHASE_C128, 0, ctypes.addressof(out)) == -1
+    assert lib.chase_filter_host_open(0x1000, 64, 0, binding.CHASE_C128, 0, ctypes.addressof(out)) == -1
+    assert lib.chase_filter_host_open(0x1000, 64, 8, 7, 0, ctypes.addressof(out)) == -4
+    assert lib.chase_filter_host_run(None, 0x1000, 4, 0x2000, -1.0, 1.0, -2.0) == -1
+    assert lib.chase_filter_host_close(None) == -1

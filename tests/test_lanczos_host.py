@@ -58,3 +58,24 @@ def test_validation():
         pkg.chase_spectral_estimates(al, bad, 50, 10)
     assert pkg.chase_lanczos_workspace_bytes(0, 5, 25, __import__("torch").float64) == 0
     assert pkg.chase_lanczos_workspace_bytes(100, 5, 25, __import__("torch").complex128) >= 100 * 5 * 26 * 16
+
+
+def test_ritz_vectors_reject_duplicate_destination_columns():
+    """Two Ritz vectors aimed at one column of V^ would race in the kernel: refused before any CUDA call
+    (fake device pointers, never dereferenced)."""
+    import numpy as np
+    lib = pkg.load()
+    k, nruns, N = 6, 2, 64
+    al, be = _coeffs(N, k, nruns, 1)
+    al, be = np.ascontiguousarray(al), np.ascontiguousarray(be)
+    cnt = np.zeros(1, dtype=np.int64)
+    wsb = pkg.chase_lanczos_workspace_bytes(N, nruns, k, __import__("torch").float64)
+
+    def call(dst):
+        d = np.asarray(dst, dtype=np.int64)
+        return lib.chase_lanczos_ritz_vectors(0x1000, wsb, N, nruns, k, 1, 1, al.ctypes.data, be.ctypes.data, -1e9,
+                                              0x2000, 8, d.ctypes.data, d.size, cnt.ctypes.data, None, None)
+
+    assert call([1, 3, 1]) == -1
+    assert call([1, 3, 8]) == -1                 # out of range
+    assert call([1, 3, 5]) == 0 and cnt[0] == 0  # mu_ne below every Ritz value: nothing written, nothing launched
