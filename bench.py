@@ -54,6 +54,8 @@ NCU_TRAFFIC = {
                                    "captures); from profiles/ncu_r2_step_dmma.md, not measured in this run"),
     5: (134.158879e9 + 1.454750e9, "bytes of one full-width launch (3000 columns; algorithmic 28.8e9 + vectors); "
                                    "from profiles/ncu_r2_step_tf32.md, not measured in this run"),
+    3: (9.788422e9 + 0.232516e9, "bytes of one full-width launch (1400 columns; algorithmic 3.2e9 + 0.45e9 of vectors); "
+                                 "from profiles/ncu_r3_step_dmma_f64.md, not measured in this run"),
     2: (328.881152e6 + 18.007808e6, "bytes of one full-width launch (256 columns; algorithmic 268e6 + vectors); "
                                     "from profiles/ncu_r2_step_dmma.md, not measured in this run"),
 }
@@ -487,6 +489,8 @@ def run_other_configs(pkg, device, headline_cfg: int):
 # (kernel path 0): one large odd-N shape per precision, so that this path has a driver-observed throughput and a
 # fraction of ITS roofline, the FP64 / FP32 FMA pipe: 148 SMs x 64 (128) FMA lanes x 2 flop x the max SM clock.
 FMA_FALLBACK_SHAPES = {"f64_N20001": (3, 20001, 700), "c64_N30001": (5, 30001, 750)}
+# dram bytes of one launch at exactly these shapes, from profiles/ncu_r3_step_generic.md (typed in, not measured here)
+FMA_FALLBACK_TRAFFIC = {"f64_N20001": 30.101692e9 + 0.112300e9, "c64_N30001": 88.987575e9 + 0.190287e9}
 
 
 def run_fma_fallback(pkg, device, sm_max_mhz: float):
@@ -507,7 +511,9 @@ def run_fma_fallback(pkg, device, sm_max_mhz: float):
                 "kernel_path": path, "value": tflops * 1e3, "unit": UNIT, "steps": steps, "warmup": 3,
                 "ms_per_step": r["dev_s"] / steps * 1e3, "dtype": DTYPE_LABEL[w.dtype],
                 "roofline": {"bound": "alu", "kernel": "step_generic_kernel", "achieved": tflops, "peak": peak,
-                             "unit": "TFLOP/s", "frac": tflops / peak, "traffic": None,
+                             "unit": "TFLOP/s", "frac": tflops / peak, "traffic": FMA_FALLBACK_TRAFFIC.get(name),
+                             "traffic_note": "bytes of one launch; from profiles/ncu_r3_step_generic.md, not measured "
+                                             "in this run",
                              "peak_source": f"148 SMs x {lanes} FMA lanes x 2 flop x {sm_max_mhz:.0f} MHz"},
                 "clocks": r["clocks"], "gpu_launches": r["launches"],
                 "rel_fro_vs_oracle": par["rel_fro_vs_oracle"], "parity": par,
